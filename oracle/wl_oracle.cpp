@@ -1,0 +1,543 @@
+// wl_oracle.cpp — CPU ORACLE for the pressure-projection path.  TEST INFRASTRUCTURE ONLY.
+//
+// A plain, slow, single-threaded C++17 statement of what the hot path computes, written from the
+// paper (/root/reference/PAPER.md, cited as PAPER.md:N) and the problem statement in
+// BASELINE.json `north_star` (cited as BJ "..."), before any CUDA kernel existed.  It shares no
+// code, header, table or helper with the CUDA library under paper_2304_08159_b200/csrc and
+// neither includes the other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may load it.  Build: g++ -O2 -ffp-contract=off -shared -fPIC (no FMA
+// contraction, IEEE division).
+//
+// Parity status of each function (what pins it other than itself: tests/test_oracle_*.py):
+//   apply_A        pinned: Kronecker-sum Neumann Laplacian (uniform L), -G^T diag(L) G incidence
+//                  form (variable L), symmetry, negative semi-definiteness, A·1 = 0, diag = -D,
+//                  cosine eigenvectors with the closed-form eigenvalue.
+//   coarsen, restrict_sum, prolong_add
+//                  pinned: dense R = P^T and A_c = R·A·P on tiny grids, uniform L -> 2^(n-1),
+//                  dyadic-rational L exact in any order.
+//   jacobi         pinned: dense x + w D^-1 (A x - b) with the pinned dense A.
+//   vcycle         pinned as far as anything external can: dense-matrix multigrid recursion built
+//                  in NumPy from the pinned A, R, P (tests/test_oracle_cycle.py).  The cycle's
+//                  constants (w = 2/3, 2+2 sweeps, 64 coarse sweeps) are fixed by BJ's text only:
+//                  no published value exists for them -> "parity unpinned" by any external number.
+//   solve          pinned: converges to the dense pseudo-inverse solution (8^2, 8^3, 12x8, 16^2
+//                  with a body) and to the cosine closed form; monotone residual history.
+//   divergence, gradient_correct, project
+//                  pinned: div(u_out) == b - A p to rounding; max|div u_out| <= tol·max|b| when
+//                  converged; -G^T / G incidence forms.
+//
+// Notation: n = ndim in {2,3}; N = (N_0..N_{n-1}), axis 0 unit-stride; cell I has
+// linear index I_0 + N_0 (I_1 + N_1 I_2); face (I,i) is the LOWER face of cell I in direction i
+// (coeff[I,i] multiplies p[I]-p[I-del(i)]).  L, u are n cell-sized fields back to
+// back (component slowest).  The upper wall face I_i = N_i is not stored and has L = 0, u = 0.
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct Dims {
+    int n;
+    int64_t N[3];
+    int64_t stride[3];
+    int64_t M;
+};
+
+Dims make_dims(int n, const int64_t* d) {
+    Dims g;
+    g.n = n;
+    for (int i = 0; i < 3; ++i) g.N[i] = (i < n) ? d[i] : 1;
+    g.stride[0] = 1;
+    g.stride[1] = g.N[0];
+    g.stride[2] = g.N[0] * g.N[1];
+    g.M = g.N[0] * g.N[1] * g.N[2];
+    return g;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Operator.  BJ "Problem statement":
+//   (A p)_I = sum_i [ L[I+di,i] (p[I+di] - p[I]) + L[I,i] (p[I-di] - p[I]) ],
+// L = 0 on domain-boundary faces (Neumann); an out-of-range neighbour is never read.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+T apply_A_cell(const Dims& g, const T* L, const T* x, int64_t I0, int64_t I1, int64_t I2) {
+    const int64_t Ii[3] = {I0, I1, I2};
+    const int64_t I = I0 + g.N[0] * (I1 + g.N[1] * I2);
+    T s = 0;
+    for (int i = 0; i < g.n; ++i) {
+        const T* Li = L + (int64_t)i * g.M;
+        if (Ii[i] + 1 < g.N[i]) s += Li[I + g.stride[i]] * (x[I + g.stride[i]] - x[I]);
+        if (Ii[i] > 0) s += Li[I] * (x[I - g.stride[i]] - x[I]);
+    }
+    return s;
+}
+
+// D_I = sum_i (L[I,i] + L[I+di,i]) = -diag(A)
+template <class T>
+T diag_cell(const Dims& g, const T* L, int64_t I0, int64_t I1, int64_t I2) {
+    const int64_t Ii[3] = {I0, I1, I2};
+    const int64_t I = I0 + g.N[0] * (I1 + g.N[1] * I2);
+    T D = 0;
+    for (int i = 0; i < g.n; ++i) {
+        const T* Li = L + (int64_t)i * g.M;
+        T Lm = (Ii[i] > 0) ? Li[I] : (T)0;
+        T Lp = (Ii[i] + 1 < g.N[i]) ? Li[I + g.stride[i]] : (T)0;
+        D += Lm + Lp;
+    }
+    return D;
+}
+
+template <class T>
+void apply_A(const Dims& g, const T* L, const T* x, T* y) {
+    for (int64_t I2 = 0; I2 < g.N[2]; ++I2)
+        for (int64_t I1 = 0; I1 < g.N[1]; ++I1)
+            for (int64_t I0 = 0; I0 < g.N[0]; ++I0)
+                y[I0 + g.N[0] * (I1 + g.N[1] * I2)] = apply_A_cell(g, L, x, I0, I1, I2);
+}
+
+// r = b - A x
+template <class T>
+void residual(const Dims& g, const T* L, const T* x, const T* b, T* r) {
+    for (int64_t I2 = 0; I2 < g.N[2]; ++I2)
+        for (int64_t I1 = 0; I1 < g.N[1]; ++I1)
+            for (int64_t I0 = 0; I0 < g.N[0]; ++I0) {
+                int64_t I = I0 + g.N[0] * (I1 + g.N[1] * I2);
+                r[I] = b[I] - apply_A_cell(g, L, x, I0, I1, I2);
+            }
+}
+
+template <class T>
+double max_abs(const T* v, int64_t M) {
+    double m = 0;
+    for (int64_t I = 0; I < M; ++I) {
+        double a = std::fabs((double)v[I]);
+        if (a > m) m = a;
+    }
+    return m;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Smoother.  BJ "Smoother: damped Jacobi, w = 2/3": every cell from the OLD x,
+//   x_new = x + w invD (A x - b),  invD = D > 0 ? 1/D : 0   (diag(A) = -D; c-7, c-10).
+// ---------------------------------------------------------------------------------------------
+template <class T>
+void jacobi_sweep(const Dims& g, const T* L, const T* x, const T* b, T* xnew) {
+    const T omega = (T)(2.0 / 3.0);
+    for (int64_t I2 = 0; I2 < g.N[2]; ++I2)
+        for (int64_t I1 = 0; I1 < g.N[1]; ++I1)
+            for (int64_t I0 = 0; I0 < g.N[0]; ++I0) {
+                int64_t I = I0 + g.N[0] * (I1 + g.N[1] * I2);
+                T D = diag_cell(g, L, I0, I1, I2);
+                T invD = (D > (T)0) ? (T)1 / D : (T)0;
+                T Ax = apply_A_cell(g, L, x, I0, I1, I2);
+                xnew[I] = x[I] + omega * invD * (Ax - b[I]);
+            }
+}
+
+template <class T>
+void jacobi(const Dims& g, const T* L, T* x, const T* b, int sweeps, std::vector<T>& tmp) {
+    tmp.resize((size_t)g.M);
+    for (int s = 0; s < sweeps; ++s) {
+        jacobi_sweep(g, L, x, b, tmp.data());
+        std::memcpy(x, tmp.data(), sizeof(T) * (size_t)g.M);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Transfers.  BJ "Restriction R sums the 2^n children; prolongation P is piecewise-constant
+// injection"; "A coarse face coefficient is the sum of the 2^(n-1) fine face coefficients
+// crossing it, so A_c = R·A·P exactly".
+// ---------------------------------------------------------------------------------------------
+template <class T>
+void restrict_sum(const Dims& gf, const Dims& gc, const T* rf, T* rc) {
+    for (int64_t J2 = 0; J2 < gc.N[2]; ++J2)
+        for (int64_t J1 = 0; J1 < gc.N[1]; ++J1)
+            for (int64_t J0 = 0; J0 < gc.N[0]; ++J0) {
+                // children 2J + c, c in {0,1}^n; summed pairwise along axis 0, then 1, then 2 (c-12)
+                T s2[2] = {0, 0};
+                int n2 = (gf.n > 2) ? 2 : 1;
+                for (int c2 = 0; c2 < n2; ++c2) {
+                    T s1[2];
+                    for (int c1 = 0; c1 < 2; ++c1) {
+                        int64_t I = (2 * J0) + gf.N[0] * ((2 * J1 + c1) + gf.N[1] * ((gf.n > 2 ? 2 * J2 : 0) + c2));
+                        s1[c1] = rf[I] + rf[I + 1];
+                    }
+                    s2[c2] = s1[0] + s1[1];
+                }
+                rc[J0 + gc.N[0] * (J1 + gc.N[1] * J2)] = (gf.n > 2) ? (s2[0] + s2[1]) : s2[0];
+            }
+}
+
+template <class T>
+void prolong_add(const Dims& gf, const Dims& gc, const T* xc, T* xf) {
+    for (int64_t I2 = 0; I2 < gf.N[2]; ++I2)
+        for (int64_t I1 = 0; I1 < gf.N[1]; ++I1)
+            for (int64_t I0 = 0; I0 < gf.N[0]; ++I0) {
+                int64_t J2 = (gf.n > 2) ? I2 / 2 : 0;
+                xf[I0 + gf.N[0] * (I1 + gf.N[1] * I2)] += xc[(I0 / 2) + gc.N[0] * ((I1 / 2) + gc.N[1] * J2)];
+            }
+}
+
+// Lc[i][J] = sum over the 2^(n-1) fine faces of direction i lying in coarse face (J,i):
+// fine cells 2J + c with c_i = 0.  n = 3, tangential axes j < k: (c_j=0,c_k=0 + c_j=1,c_k=0) +
+// (c_j=0,c_k=1 + c_j=1,c_k=1)  (fixed tree, c-12: the CUDA kernel must be bit-exact against this).
+template <class T>
+void coarsen(const Dims& gf, const Dims& gc, const T* Lf, T* Lc) {
+    for (int i = 0; i < gf.n; ++i) {
+        const T* Lfi = Lf + (int64_t)i * gf.M;
+        T* Lci = Lc + (int64_t)i * gc.M;
+        int tj = -1, tk = -1;  // tangential axes, ascending
+        for (int a = 0; a < gf.n; ++a)
+            if (a != i) { if (tj < 0) tj = a; else tk = a; }
+        for (int64_t J2 = 0; J2 < gc.N[2]; ++J2)
+            for (int64_t J1 = 0; J1 < gc.N[1]; ++J1)
+                for (int64_t J0 = 0; J0 < gc.N[0]; ++J0) {
+                    const int64_t J[3] = {J0, J1, J2};
+                    int64_t base = 0;
+                    for (int a = 0; a < gf.n; ++a) base += 2 * J[a] * gf.stride[a];
+                    T s;
+                    if (gf.n == 2) {
+                        s = Lfi[base] + Lfi[base + gf.stride[tj]];
+                    } else {
+                        T a0 = Lfi[base] + Lfi[base + gf.stride[tj]];
+                        T a1 = Lfi[base + gf.stride[tk]] + Lfi[base + gf.stride[tj] + gf.stride[tk]];
+                        s = a0 + a1;
+                    }
+                    Lci[J0 + gc.N[0] * (J1 + gc.N[1] * J2)] = s;
+                }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// H1 divergence: b[I] = sum_i (u[i][I+di] - u[i][I]); unstored upper wall face = 0.
+// (BJ "Fused divergence"; configs[0] "b = sum_i (L u)[I+di,i] - (L u)[I,i]" with the masked
+//  velocity passed in.)
+// H8 gradient correction: u[i][I] -= L[i][I] (p[I] - p[I-di]); plane I_i = 0
+// untouched (its L is 0 and p[I-di] does not exist).
+// ---------------------------------------------------------------------------------------------
+template <class T>
+void divergence(const Dims& g, const T* u, T* b) {
+    for (int64_t I2 = 0; I2 < g.N[2]; ++I2)
+        for (int64_t I1 = 0; I1 < g.N[1]; ++I1)
+            for (int64_t I0 = 0; I0 < g.N[0]; ++I0) {
+                const int64_t Ii[3] = {I0, I1, I2};
+                int64_t I = I0 + g.N[0] * (I1 + g.N[1] * I2);
+                T s = 0;
+                for (int i = 0; i < g.n; ++i) {
+                    const T* ui = u + (int64_t)i * g.M;
+                    T up = (Ii[i] + 1 < g.N[i]) ? ui[I + g.stride[i]] : (T)0;
+                    s += up - ui[I];
+                }
+                b[I] = s;
+            }
+}
+
+template <class T>
+void gradient_correct(const Dims& g, const T* L, T* u, const T* p) {
+    for (int i = 0; i < g.n; ++i) {
+        const T* Li = L + (int64_t)i * g.M;
+        T* ui = u + (int64_t)i * g.M;
+        for (int64_t I2 = 0; I2 < g.N[2]; ++I2)
+            for (int64_t I1 = 0; I1 < g.N[1]; ++I1)
+                for (int64_t I0 = 0; I0 < g.N[0]; ++I0) {
+                    const int64_t Ii[3] = {I0, I1, I2};
+                    if (Ii[i] == 0) continue;
+                    int64_t I = I0 + g.N[0] * (I1 + g.N[1] * I2);
+                    ui[I] -= Li[I] * (p[I] - p[I - g.stride[i]]);
+                }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Hierarchy + V-cycle + solve + project (SURVEY.md §8(c) "Algorithm", each line from BJ).
+// ---------------------------------------------------------------------------------------------
+template <class T>
+struct Level {
+    Dims g;
+    std::vector<T> L;  // n*M
+    std::vector<T> x, b;  // levels >= 1 only
+};
+
+template <class T>
+struct Ctx {
+    int n;
+    std::vector<Level<T>> lev;  // lev[0] = finest
+    std::vector<T> tmp, r;
+    bool have_coeff = false;
+};
+
+// BJ "The hierarchy halves every dimension down to a 4^n grid"; for general dims: coarsen while
+// every extent is even and every half is >= 4 (c-4).
+int num_coarsenings(int n, const int64_t* d) {
+    int k = 0;
+    int64_t N[3] = {d[0], d[1], n > 2 ? d[2] : 1};
+    while (true) {
+        bool ok = true;
+        for (int i = 0; i < n; ++i)
+            if (N[i] % 2 != 0 || N[i] / 2 < 4) ok = false;
+        if (!ok) break;
+        for (int i = 0; i < n; ++i) N[i] /= 2;
+        ++k;
+    }
+    return k;
+}
+
+template <class T>
+Ctx<T>* ctx_create(int n, const int64_t* d) {
+    Ctx<T>* c = new Ctx<T>();
+    c->n = n;
+    int K = num_coarsenings(n, d);
+    int64_t N[3] = {d[0], d[1], n > 2 ? d[2] : 1};
+    for (int l = 0; l <= K; ++l) {
+        Level<T> lv;
+        lv.g = make_dims(n, N);
+        lv.L.assign((size_t)(n * lv.g.M), (T)0);
+        if (l > 0) {
+            lv.x.assign((size_t)lv.g.M, (T)0);
+            lv.b.assign((size_t)lv.g.M, (T)0);
+        }
+        c->lev.push_back(std::move(lv));
+        for (int i = 0; i < n; ++i) N[i] /= 2;
+    }
+    return c;
+}
+
+// H0: level 0 = copy of the caller's L with the stored wall plane I_i = 0 forced to 0 (c-6); then
+// one coarsening per level.
+template <class T>
+void ctx_set_coeff(Ctx<T>* c, const T* L) {
+    Level<T>& f = c->lev[0];
+    std::memcpy(f.L.data(), L, sizeof(T) * (size_t)(c->n * f.g.M));
+    for (int i = 0; i < c->n; ++i)
+        for (int64_t I2 = 0; I2 < f.g.N[2]; ++I2)
+            for (int64_t I1 = 0; I1 < f.g.N[1]; ++I1)
+                for (int64_t I0 = 0; I0 < f.g.N[0]; ++I0) {
+                    const int64_t Ii[3] = {I0, I1, I2};
+                    if (Ii[i] == 0) f.L[(size_t)(i * f.g.M + I0 + f.g.N[0] * (I1 + f.g.N[1] * I2))] = (T)0;
+                }
+    for (size_t l = 0; l + 1 < c->lev.size(); ++l)
+        coarsen(c->lev[l].g, c->lev[l + 1].g, c->lev[l].L.data(), c->lev[l + 1].L.data());
+    c->have_coeff = true;
+}
+
+// VCYCLE(l) on (x, b) of level l.
+template <class T>
+void vcycle(Ctx<T>* c, size_t l, T* x, const T* b) {
+    Level<T>& lv = c->lev[l];
+    const size_t last = c->lev.size() - 1;
+    if (l == last) {
+        // BJ "The coarsest level gets 64 Jacobi sweeps" (from x = 0 when it is a correction level;
+        // with no coarsening at all the "cycle" is 64 sweeps from the current iterate)
+        if (last > 0) std::fill(x, x + lv.g.M, (T)0);
+        jacobi(lv.g, lv.L.data(), x, b, 64, c->tmp);
+        return;
+    }
+    Level<T>& cv = c->lev[l + 1];
+    jacobi(lv.g, lv.L.data(), x, b, 2, c->tmp);                        // BJ "2 pre-sweeps"
+    std::vector<T> r((size_t)lv.g.M);
+    residual(lv.g, lv.L.data(), x, b, r.data());                       // r = b - A x
+    restrict_sum(lv.g, cv.g, r.data(), cv.b.data());                   // b_c = R r
+    std::fill(cv.x.begin(), cv.x.end(), (T)0);                         // x_c = 0 (c-11)
+    vcycle(c, l + 1, cv.x.data(), cv.b.data());
+    prolong_add(lv.g, cv.g, cv.x.data(), x);                           // x += P x_c
+    jacobi(lv.g, lv.L.data(), x, b, 2, c->tmp);                        // BJ "2 post-sweeps"
+}
+
+// p -= mean(p): sum in fp64 over all cells, subtract (T)mean (c-13).
+template <class T>
+void remove_mean(T* p, int64_t M) {
+    double s = 0;
+    for (int64_t I = 0; I < M; ++I) s += (double)p[I];
+    T m = (T)(s / (double)M);
+    for (int64_t I = 0; I < M; ++I) p[I] -= m;
+}
+
+template <class T>
+double resnorm(Ctx<T>* c, const T* p, const T* b) {
+    Level<T>& f = c->lev[0];
+    c->r.resize((size_t)f.g.M);
+    residual(f.g, f.L.data(), p, b, c->r.data());
+    return max_abs(c->r.data(), f.g.M);
+}
+
+// One VCYCLE(0) + mean removal; returns ||b - A p||inf of the returned p.
+template <class T>
+double ctx_vcycle(Ctx<T>* c, T* p, const T* b) {
+    vcycle(c, 0, p, b);
+    remove_mean(p, c->lev[0].g.M);
+    return resnorm(c, p, b);
+}
+
+// SOLVE (BJ "V-cycles repeat until ||r||inf <= 1e-4 ||b||inf or 32 cycles"): hist[0] before any
+// cycle, hist[k] after k (c-14).  Returns 0 if converged, 1 if the cycle cap was reached.
+template <class T>
+int ctx_solve(Ctx<T>* c, T* p, const T* b, double tol, int maxcycles, double* hist, int* ncycles) {
+    const int64_t M = c->lev[0].g.M;
+    double nb = max_abs(b, M);
+    hist[0] = resnorm(c, p, b);
+    int k = 0;
+    while (k < maxcycles && hist[k] > tol * nb) {
+        hist[k + 1] = ctx_vcycle(c, p, b);
+        ++k;
+    }
+    if (k == 0) remove_mean(p, M);
+    *ncycles = k;
+    return (hist[k] > tol * nb) ? 1 : 0;
+}
+
+// PROJECT (PAPER.md:29-33 + BJ "wl_project(u, L, p), which computes the divergence, solves, and
+// corrects u").
+template <class T>
+int ctx_project(Ctx<T>* c, T* u, const T* L, T* p, double tol, int maxcycles, double* hist, int* ncycles) {
+    if (L) ctx_set_coeff(c, L);
+    Level<T>& f = c->lev[0];
+    std::vector<T> b((size_t)f.g.M);
+    divergence(f.g, u, b.data());
+    int rc = ctx_solve(c, p, b.data(), tol, maxcycles, hist, ncycles);
+    gradient_correct(f.g, f.L.data(), u, p);
+    return rc;
+}
+
+struct Handle {
+    int dtype;  // 0 = f32, 1 = f64
+    void* ctx;
+};
+
+}  // namespace
+
+#define DISPATCH(h, expr_f, expr_d) \
+    do { if ((h)->dtype == 0) { typedef float T; Ctx<T>* c = (Ctx<T>*)(h)->ctx; (void)c; expr_f; } \
+         else { typedef double T; Ctx<T>* c = (Ctx<T>*)(h)->ctx; (void)c; expr_d; } } while (0)
+
+extern "C" {
+
+void* orc_create(int ndim, const int64_t* dims, int dtype) {
+    if (ndim < 2 || ndim > 3 || (dtype != 0 && dtype != 1)) return nullptr;
+    for (int i = 0; i < ndim; ++i) if (dims[i] < 4) return nullptr;
+    Handle* h = new Handle();
+    h->dtype = dtype;
+    h->ctx = (dtype == 0) ? (void*)ctx_create<float>(ndim, dims) : (void*)ctx_create<double>(ndim, dims);
+    return h;
+}
+
+void orc_destroy(void* hv) {
+    Handle* h = (Handle*)hv;
+    if (!h) return;
+    if (h->dtype == 0) delete (Ctx<float>*)h->ctx; else delete (Ctx<double>*)h->ctx;
+    delete h;
+}
+
+int orc_num_levels(void* hv) {
+    Handle* h = (Handle*)hv;
+    int r = 0;
+    DISPATCH(h, r = (int)c->lev.size(), r = (int)c->lev.size());
+    return r;
+}
+
+void orc_level_dims(void* hv, int level, int64_t* out) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, for (int i = 0; i < c->n; ++i) out[i] = c->lev[level].g.N[i],
+                for (int i = 0; i < c->n; ++i) out[i] = c->lev[level].g.N[i]);
+}
+
+void orc_set_coeff(void* hv, const void* L) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, ctx_set_coeff(c, (const T*)L), ctx_set_coeff(c, (const T*)L));
+}
+
+void orc_get_coeff(void* hv, int level, void* out) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, std::memcpy(out, c->lev[level].L.data(), sizeof(T) * c->lev[level].L.size()),
+                std::memcpy(out, c->lev[level].L.data(), sizeof(T) * c->lev[level].L.size()));
+}
+
+// y = A_level x
+void orc_apply_A(void* hv, int level, const void* x, void* y) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, apply_A(c->lev[level].g, c->lev[level].L.data(), (const T*)x, (T*)y),
+                apply_A(c->lev[level].g, c->lev[level].L.data(), (const T*)x, (T*)y));
+}
+
+// r = b - A_level x ; returns ||r||inf
+double orc_residual(void* hv, int level, const void* x, const void* b, void* r) {
+    Handle* h = (Handle*)hv;
+    double m = 0;
+    DISPATCH(h, (residual(c->lev[level].g, c->lev[level].L.data(), (const T*)x, (const T*)b, (T*)r),
+                 m = max_abs((const T*)r, c->lev[level].g.M)),
+                (residual(c->lev[level].g, c->lev[level].L.data(), (const T*)x, (const T*)b, (T*)r),
+                 m = max_abs((const T*)r, c->lev[level].g.M)));
+    return m;
+}
+
+// `sweeps` damped-Jacobi sweeps on level `level`, in place on x
+void orc_jacobi(void* hv, int level, void* x, const void* b, int sweeps) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, jacobi(c->lev[level].g, c->lev[level].L.data(), (T*)x, (const T*)b, sweeps, c->tmp),
+                jacobi(c->lev[level].g, c->lev[level].L.data(), (T*)x, (const T*)b, sweeps, c->tmp));
+}
+
+// rc = R r_f (level -> level+1)
+void orc_restrict(void* hv, int level, const void* rf, void* rc) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, restrict_sum(c->lev[level].g, c->lev[level + 1].g, (const T*)rf, (T*)rc),
+                restrict_sum(c->lev[level].g, c->lev[level + 1].g, (const T*)rf, (T*)rc));
+}
+
+// x_f += P x_c (level+1 -> level)
+void orc_prolong_add(void* hv, int level, const void* xc, void* xf) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, prolong_add(c->lev[level].g, c->lev[level + 1].g, (const T*)xc, (T*)xf),
+                prolong_add(c->lev[level].g, c->lev[level + 1].g, (const T*)xc, (T*)xf));
+}
+
+// VCYCLE(level) on caller arrays of that level (no mean removal)
+void orc_vcycle_level(void* hv, int level, void* x, const void* b) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, vcycle(c, (size_t)level, (T*)x, (const T*)b), vcycle(c, (size_t)level, (T*)x, (const T*)b));
+}
+
+// one VCYCLE(0) + mean removal; returns ||b - A p||inf
+double orc_vcycle(void* hv, void* p, const void* b) {
+    Handle* h = (Handle*)hv;
+    double r = 0;
+    DISPATCH(h, r = ctx_vcycle(c, (T*)p, (const T*)b), r = ctx_vcycle(c, (T*)p, (const T*)b));
+    return r;
+}
+
+int orc_solve(void* hv, void* p, const void* b, double tol, int maxcycles, double* hist, int* ncycles) {
+    Handle* h = (Handle*)hv;
+    int rc = 0;
+    DISPATCH(h, rc = ctx_solve(c, (T*)p, (const T*)b, tol, maxcycles, hist, ncycles),
+                rc = ctx_solve(c, (T*)p, (const T*)b, tol, maxcycles, hist, ncycles));
+    return rc;
+}
+
+int orc_project(void* hv, void* u, const void* L, void* p, double tol, int maxcycles, double* hist, int* ncycles) {
+    Handle* h = (Handle*)hv;
+    int rc = 0;
+    DISPATCH(h, rc = ctx_project(c, (T*)u, (const T*)L, (T*)p, tol, maxcycles, hist, ncycles),
+                rc = ctx_project(c, (T*)u, (const T*)L, (T*)p, tol, maxcycles, hist, ncycles));
+    return rc;
+}
+
+void orc_divergence(void* hv, const void* u, void* b) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, divergence(c->lev[0].g, (const T*)u, (T*)b), divergence(c->lev[0].g, (const T*)u, (T*)b));
+}
+
+// u[i][I] -= L0[i][I] (p[I] - p[I-di]) with the ctx's level-0 coefficients
+void orc_gradient_correct(void* hv, void* u, const void* p) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, gradient_correct(c->lev[0].g, c->lev[0].L.data(), (T*)u, (const T*)p),
+                gradient_correct(c->lev[0].g, c->lev[0].L.data(), (T*)u, (const T*)p));
+}
+
+// p -= mean(p)
+void orc_remove_mean(void* hv, void* p) {
+    Handle* h = (Handle*)hv;
+    DISPATCH(h, remove_mean((T*)p, c->lev[0].g.M), remove_mean((T*)p, c->lev[0].g.M));
+}
+
+}  // extern "C"
