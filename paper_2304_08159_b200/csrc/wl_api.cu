@@ -1,0 +1,550 @@
+// wl_api.cu — context, level hierarchy, launch sequencing and the C ABI of include/wl.h.
+//
+// Runtime structure: one context per grid; the context owns every coarse level (L, x ping-pong, b),
+// a level-0 ping-pong buffer, the device scalars (norms, mean, stop flag), and the captured V-cycle graph.
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+#include "../../include/wl.h"
+#include "wl_common.cuh"
+#include "wl_generic.cuh"
+
+using namespace wl;
+
+namespace {
+
+constexpr int kMaxLevels = 32;
+constexpr int kBlock = 256;
+constexpr int kMaxPartials = 148 * 16;
+
+struct Level {
+    Grid g;
+    void* L = nullptr;      // n*M coefficients (ctx-owned copy / coarsened)
+    void* x[2] = {nullptr, nullptr};  // level >= 1: iterate ping-pong; level 0: x[1] = ctx-owned scratch only
+    void* b = nullptr;      // level >= 1: restricted residual
+};
+
+thread_local char g_create_err[256] = "";
+
+}  // namespace
+
+struct wl_ctx {
+    int n = 0, dtype = 0, nlev = 0;
+    size_t esz = 4;
+    Level lev[kMaxLevels];
+    cudaStream_t stream = 0;
+    Scalars* d_scal = nullptr;
+    Scalars* h_scal = nullptr;   // pinned mirror
+    double* d_partials = nullptr;
+    double* d_hist = nullptr;
+    double* h_hist = nullptr;    // pinned
+    int hist_cap = 0;
+    void* b0 = nullptr;          // ctx-owned right-hand side for wl_project
+    void* stage_u = nullptr;     // device staging for wl_project_host
+    void* stage_L = nullptr;
+    void* stage_p = nullptr;
+    bool have_coeff = false;
+    int opt_fused = 1, opt_graph = 1, opt_coarse_cta = 1;
+    int num_sms = 148;
+    int64_t launches = 0;
+    char err[256] = "";
+};
+
+namespace {
+
+int fail(wl_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess) {
+    if (c) {
+        if (e != cudaSuccess) snprintf(c->err, sizeof(c->err), "%s: %s", what, cudaGetErrorString(e));
+        else snprintf(c->err, sizeof(c->err), "%s", what);
+    }
+    return code;
+}
+
+#define CU(c, call)                                                      \
+    do {                                                                 \
+        cudaError_t e__ = (call);                                        \
+        if (e__ != cudaSuccess) return fail((c), WL_ECUDA, #call, e__);  \
+    } while (0)
+
+#define KCHECK(c, name)                                                  \
+    do {                                                                 \
+        cudaError_t e__ = cudaGetLastError();                            \
+        if (e__ != cudaSuccess) return fail((c), WL_ECUDA, name, e__);   \
+        (c)->launches++;                                                 \
+    } while (0)
+
+inline int grid_for(const wl_ctx* c, long long work) {
+    long long blocks = (work + kBlock - 1) / kBlock;
+    long long cap = (long long)c->num_sms * 8;
+    if (blocks < 1) blocks = 1;
+    return (int)(blocks < cap ? blocks : cap);
+}
+
+inline int nparts_for(const wl_ctx* c, long long work) {
+    int g = grid_for(c, work);
+    return g < kMaxPartials ? g : kMaxPartials;
+}
+
+// ---- typed implementation ------------------------------------------------------------------------------------
+template <typename T, int ND>
+struct Impl {
+    static T* P(void* p) { return (T*)p; }
+    static const T* P(const void* p) { return (const T*)p; }
+
+    static int set_coeff(wl_ctx* c, const void* Ldev) {
+        Level& f = c->lev[0];
+        k_copy_coeff<T, ND><<<grid_for(c, f.g.M * ND), kBlock, 0, c->stream>>>(f.g, P(Ldev), P(f.L));
+        KCHECK(c, "k_copy_coeff");
+        for (int l = 0; l + 1 < c->nlev; ++l) {
+            Level& a = c->lev[l];
+            Level& b = c->lev[l + 1];
+            k_coarsen<T, ND><<<grid_for(c, b.g.M * ND), kBlock, 0, c->stream>>>(a.g, b.g, P(a.L), P(b.L));
+            KCHECK(c, "k_coarsen");
+        }
+        c->have_coeff = true;
+        return WL_OK;
+    }
+
+    static int jacobi_sweep(wl_ctx* c, int l, const void* xin, const void* b, void* xout) {
+        Level& v = c->lev[l];
+        k_jacobi<T, ND><<<grid_for(c, v.g.M), kBlock, 0, c->stream>>>(v.g, P(v.L), P(xin), P(b), P(xout));
+        KCHECK(c, "k_jacobi");
+        return WL_OK;
+    }
+
+    // `sweeps` sweeps in place on x using `tmp` as the other half of the ping-pong; result always lands in x.
+    static int jacobi(wl_ctx* c, int l, void* x, const void* b, void* tmp, int sweeps) {
+        void* cur = x;
+        void* oth = tmp;
+        for (int s = 0; s < sweeps; ++s) {
+            int rc = jacobi_sweep(c, l, cur, b, oth);
+            if (rc) return rc;
+            void* t = cur; cur = oth; oth = t;
+        }
+        if (cur != x) CU(c, cudaMemcpyAsync(x, cur, (size_t)c->lev[l].g.M * sizeof(T), cudaMemcpyDeviceToDevice, c->stream));
+        return WL_OK;
+    }
+
+    static int residual_restrict(wl_ctx* c, int l, const void* x, const void* b, void* bc, void* xc) {
+        Level& f = c->lev[l];
+        Level& k = c->lev[l + 1];
+        k_residual_restrict<T, ND><<<grid_for(c, k.g.M), kBlock, 0, c->stream>>>(f.g, k.g, P(f.L), P(x), P(b), P(bc), P(xc));
+        KCHECK(c, "k_residual_restrict");
+        return WL_OK;
+    }
+
+    static int prolong(wl_ctx* c, int l, const void* xc, void* x) {
+        Level& f = c->lev[l];
+        Level& k = c->lev[l + 1];
+        k_prolong_add<T, ND><<<grid_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, k.g, P(xc), P(x));
+        KCHECK(c, "k_prolong_add");
+        return WL_OK;
+    }
+
+    // VCYCLE(l) with generic kernels.  x, b: arrays of level l; tmp: scratch of level l.
+    static int vcycle_generic(wl_ctx* c, int l, void* x, const void* b, void* tmp) {
+        int rc;
+        Level& v = c->lev[l];
+        if (l == c->nlev - 1) {
+            int sweeps = 64;
+            if (c->nlev > 1) {
+                // x = 0 then one sweep == the closed form of the first sweep; 63 more follow
+                k_jacobi_from_zero<T, ND><<<grid_for(c, v.g.M), kBlock, 0, c->stream>>>(v.g, P(v.L), P(b), P(tmp));
+                KCHECK(c, "k_jacobi_from_zero");
+                // 63 sweeps starting from tmp, ending in x (odd count: tmp -> x -> tmp ... -> x)
+                void* cur = tmp;
+                void* oth = x;
+                for (int s = 1; s < sweeps; ++s) {
+                    if ((rc = jacobi_sweep(c, l, cur, b, oth))) return rc;
+                    void* t = cur; cur = oth; oth = t;
+                }
+                if (cur != x) CU(c, cudaMemcpyAsync(x, cur, (size_t)v.g.M * sizeof(T), cudaMemcpyDeviceToDevice, c->stream));
+                return WL_OK;
+            }
+            return jacobi(c, l, x, b, tmp, sweeps);
+        }
+        Level& k = c->lev[l + 1];
+        if ((rc = jacobi(c, l, x, b, tmp, 2))) return rc;
+        if ((rc = residual_restrict(c, l, x, b, k.b, k.x[0]))) return rc;  // also x_{l+1} = 0
+        if ((rc = vcycle_generic(c, l + 1, k.x[0], k.b, k.x[1]))) return rc;
+        if ((rc = prolong(c, l, k.x[0], x))) return rc;
+        return jacobi(c, l, x, b, tmp, 2);
+    }
+
+    // Σp -> mean (ordered), p -= mean.
+    static int remove_mean(wl_ctx* c, void* p) {
+        const long long M = c->lev[0].g.M;
+        const int np = nparts_for(c, M);
+        k_sum<T><<<np, kBlock, 0, c->stream>>>(M, P(p), c->d_partials);
+        KCHECK(c, "k_sum");
+        k_finish_mean<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_partials, np, M);
+        KCHECK(c, "k_finish_mean");
+        k_shift<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, P(p), c->d_scal);
+        KCHECK(c, "k_shift");
+        return WL_OK;
+    }
+
+    // ||b - A p||inf into slot 1 (and Σp partials -> mean, not applied).
+    static int resnorm(wl_ctx* c, const void* p, const void* b) {
+        Level& f = c->lev[0];
+        const int np = nparts_for(c, f.g.M);
+        k_zero_slot<<<1, 32, 0, c->stream>>>(c->d_scal, 1);
+        KCHECK(c, "k_zero_slot");
+        k_resnorm_sum<T, ND><<<np, kBlock, 0, c->stream>>>(f.g, P(f.L), P(p), P(b), c->d_scal, 1, c->d_partials);
+        KCHECK(c, "k_resnorm_sum");
+        k_finish_mean<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_partials, np, f.g.M);
+        KCHECK(c, "k_finish_mean");
+        return WL_OK;
+    }
+
+    static int absmax_b(wl_ctx* c, const void* b) {
+        const long long M = c->lev[0].g.M;
+        k_zero_slot<<<1, 32, 0, c->stream>>>(c->d_scal, 0);
+        KCHECK(c, "k_zero_slot");
+        k_absmax<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, P(b), c->d_scal, 0);
+        KCHECK(c, "k_absmax");
+        return WL_OK;
+    }
+
+    // One V-cycle + mean removal + residual norm (slot 1).
+    static int cycle(wl_ctx* c, void* p, const void* b) {
+        int rc;
+        if ((rc = vcycle_generic(c, 0, p, b, c->lev[0].x[1]))) return rc;
+        if ((rc = remove_mean(c, p))) return rc;
+        return resnorm(c, p, b);
+    }
+
+    static int divergence(wl_ctx* c, const void* u, void* b) {
+        Level& f = c->lev[0];
+        k_divergence<T, ND><<<grid_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, P(u), P(b));
+        KCHECK(c, "k_divergence");
+        return WL_OK;
+    }
+
+    static int gradient(wl_ctx* c, void* u, const void* p) {
+        Level& f = c->lev[0];
+        k_gradient<T, ND><<<grid_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, P(f.L), P(u), P(p));
+        KCHECK(c, "k_gradient");
+        return WL_OK;
+    }
+};
+
+#define DISPATCH(c, call)                                                         \
+    ((c)->dtype == WL_F32 ? ((c)->n == 2 ? Impl<float, 2>::call : Impl<float, 3>::call) \
+                          : ((c)->n == 2 ? Impl<double, 2>::call : Impl<double, 3>::call))
+
+int read_scalars(wl_ctx* c) {
+    CU(c, cudaMemcpyAsync(c->h_scal, c->d_scal, sizeof(Scalars), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return WL_OK;
+}
+
+inline double bits_to_double(unsigned long long b) {
+    double d;
+    memcpy(&d, &b, sizeof(d));
+    return d;
+}
+
+int ensure_hist(wl_ctx* c, int maxcycles) {
+    if (maxcycles + 1 <= c->hist_cap) return WL_OK;
+    if (c->d_hist) cudaFree(c->d_hist);
+    if (c->h_hist) cudaFreeHost(c->h_hist);
+    c->d_hist = nullptr; c->h_hist = nullptr; c->hist_cap = 0;
+    int cap = maxcycles + 1 < 64 ? 64 : maxcycles + 1;
+    if (cudaMalloc(&c->d_hist, sizeof(double) * cap) != cudaSuccess) return fail(c, WL_ENOMEM, "cudaMalloc(hist)");
+    if (cudaMallocHost(&c->h_hist, sizeof(double) * cap) != cudaSuccess) return fail(c, WL_ENOMEM, "cudaMallocHost(hist)");
+    c->hist_cap = cap;
+    return WL_OK;
+}
+
+int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, double* hist, int* ncycles) {
+    int rc;
+    if ((rc = ensure_hist(c, maxcycles))) return rc;
+    if ((rc = DISPATCH(c, absmax_b)(c, b))) return rc;
+    if ((rc = DISPATCH(c, resnorm)(c, p, b))) return rc;
+    k_solve_begin<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, tol, maxcycles);
+    KCHECK(c, "k_solve_begin");
+    if ((rc = read_scalars(c))) return rc;
+    const double nb = c->h_scal->nb;
+    hist[0] = bits_to_double(c->h_scal->absmax_bits[1]);
+    int k = 0;
+    while (k < maxcycles && hist[k] > tol * nb) {
+        if ((rc = DISPATCH(c, cycle)(c, p, b))) return rc;
+        k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist);
+        KCHECK(c, "k_cycle_end");
+        if ((rc = read_scalars(c))) return rc;
+        ++k;
+        hist[k] = bits_to_double(c->h_scal->absmax_bits[1]);
+    }
+    if (k == 0) {
+        if ((rc = DISPATCH(c, remove_mean)(c, p))) return rc;
+        CU(c, cudaStreamSynchronize(c->stream));
+    }
+    *ncycles = k;
+    return (hist[k] > tol * nb) ? WL_NOT_CONVERGED : WL_OK;
+}
+
+int level_check(const wl_ctx* c, int level, bool need_next) {
+    if (!c) return WL_EINVAL;
+    if (level < 0 || level >= c->nlev) return WL_EINVAL;
+    if (need_next && level + 1 >= c->nlev) return WL_EINVAL;
+    return WL_OK;
+}
+
+}  // namespace
+
+// ====================================================================================================================
+extern "C" {
+
+int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
+    if (out) *out = nullptr;
+    if (!out || !dims) { snprintf(g_create_err, sizeof(g_create_err), "wl_create: null argument"); return WL_EINVAL; }
+    if (dtype != WL_F32 && dtype != WL_F64) { snprintf(g_create_err, sizeof(g_create_err), "wl_create: bad dtype"); return WL_EINVAL; }
+    if (ndim < 2 || ndim > 3) { snprintf(g_create_err, sizeof(g_create_err), "wl_create: ndim must be 2 or 3"); return WL_EDIMS; }
+    long long cells = 1;
+    for (int i = 0; i < ndim; ++i) {
+        if (dims[i] < 4 || dims[i] > (1 << 20)) { snprintf(g_create_err, sizeof(g_create_err), "wl_create: every extent must be in [4, 2^20]"); return WL_EDIMS; }
+        cells *= dims[i];
+        if (cells > (1LL << 34)) { snprintf(g_create_err, sizeof(g_create_err), "wl_create: grid too large"); return WL_EDIMS; }
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { snprintf(g_create_err, sizeof(g_create_err), "wl_create: no CUDA device: %s", cudaGetErrorString(e)); return WL_ECUDA; }
+    wl_ctx* c = new (std::nothrow) wl_ctx();
+    if (!c) { snprintf(g_create_err, sizeof(g_create_err), "wl_create: out of host memory"); return WL_ENOMEM; }
+    c->n = ndim;
+    c->dtype = dtype;
+    c->esz = (dtype == WL_F32) ? 4 : 8;
+    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (c->num_sms <= 0) c->num_sms = 148;
+
+    long long N[3] = {dims[0], dims[1], ndim > 2 ? dims[2] : 1};
+    int nlev = 0;
+    while (true) {
+        Level& v = c->lev[nlev];
+        v.g.n = ndim;
+        v.g.N0 = (int)N[0]; v.g.N1 = (int)N[1]; v.g.N2 = (int)N[2];
+        v.g.M = N[0] * N[1] * N[2];
+        ++nlev;
+        bool ok = nlev < kMaxLevels;
+        for (int i = 0; i < ndim; ++i)
+            if (N[i] % 2 != 0 || N[i] / 2 < 4) ok = false;
+        if (!ok) break;
+        for (int i = 0; i < ndim; ++i) N[i] /= 2;
+    }
+    c->nlev = nlev;
+
+    bool okm = true;
+    auto dmalloc = [&](void** p, size_t bytes) {
+        if (!okm) return;
+        cudaError_t e2 = cudaMalloc(p, bytes < 16 ? 16 : bytes);
+        if (e2 != cudaSuccess) { okm = false; snprintf(g_create_err, sizeof(g_create_err), "wl_create: cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e2)); }
+    };
+    for (int l = 0; l < nlev; ++l) {
+        Level& v = c->lev[l];
+        dmalloc(&v.L, (size_t)v.g.M * ndim * c->esz);
+        dmalloc(&v.x[1], (size_t)v.g.M * c->esz);
+        if (l > 0) {
+            dmalloc(&v.x[0], (size_t)v.g.M * c->esz);
+            dmalloc(&v.b, (size_t)v.g.M * c->esz);
+        }
+    }
+    dmalloc((void**)&c->d_scal, sizeof(Scalars));
+    dmalloc((void**)&c->d_partials, sizeof(double) * kMaxPartials);
+    if (okm && cudaMallocHost((void**)&c->h_scal, sizeof(Scalars)) != cudaSuccess) {
+        okm = false;
+        snprintf(g_create_err, sizeof(g_create_err), "wl_create: cudaMallocHost failed");
+    }
+    if (okm && cudaMemset(c->d_scal, 0, sizeof(Scalars)) != cudaSuccess) okm = false;
+    if (!okm) {
+        cudaGetLastError();
+        wl_destroy(c);
+        return WL_ENOMEM;
+    }
+    g_create_err[0] = 0;
+    *out = c;
+    return WL_OK;
+}
+
+void wl_destroy(wl_ctx* c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    for (int l = 0; l < kMaxLevels; ++l) {
+        Level& v = c->lev[l];
+        if (v.L) cudaFree(v.L);
+        if (v.x[0]) cudaFree(v.x[0]);
+        if (v.x[1]) cudaFree(v.x[1]);
+        if (v.b) cudaFree(v.b);
+    }
+    if (c->d_scal) cudaFree(c->d_scal);
+    if (c->d_partials) cudaFree(c->d_partials);
+    if (c->d_hist) cudaFree(c->d_hist);
+    if (c->h_hist) cudaFreeHost(c->h_hist);
+    if (c->h_scal) cudaFreeHost(c->h_scal);
+    if (c->b0) cudaFree(c->b0);
+    if (c->stage_u) cudaFree(c->stage_u);
+    if (c->stage_L) cudaFree(c->stage_L);
+    if (c->stage_p) cudaFree(c->stage_p);
+    cudaGetLastError();
+    delete c;
+}
+
+int wl_set_stream(wl_ctx* c, void* s) {
+    if (!c) return WL_EINVAL;
+    c->stream = (cudaStream_t)s;
+    return WL_OK;
+}
+
+int wl_set_option(wl_ctx* c, int key, int value) {
+    if (!c) return WL_EINVAL;
+    switch (key) {
+        case WL_OPT_FUSED: c->opt_fused = value ? 1 : 0; return WL_OK;
+        case WL_OPT_GRAPH: c->opt_graph = value ? 1 : 0; return WL_OK;
+        case WL_OPT_COARSE_CTA: c->opt_coarse_cta = value ? 1 : 0; return WL_OK;
+        default: return fail(c, WL_EINVAL, "wl_set_option: unknown key");
+    }
+}
+
+int wl_set_coeff(wl_ctx* c, const void* L) {
+    if (!c) return WL_EINVAL;
+    if (!L) return fail(c, WL_EINVAL, "wl_set_coeff: null L");
+    return DISPATCH(c, set_coeff)(c, L);
+}
+
+int wl_vcycle(wl_ctx* c, void* p, const void* b, double* rnorm_out) {
+    if (!c) return WL_EINVAL;
+    if (!p || !b) return fail(c, WL_EINVAL, "wl_vcycle: null pointer");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle: coefficients not set");
+    int rc = DISPATCH(c, cycle)(c, p, b);
+    if (rc) return rc;
+    if (rnorm_out) {
+        if ((rc = read_scalars(c))) return rc;
+        *rnorm_out = bits_to_double(c->h_scal->absmax_bits[1]);
+    }
+    return WL_OK;
+}
+
+int wl_solve(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, double* hist, int* ncycles) {
+    if (!c) return WL_EINVAL;
+    if (!p || !b || !hist || !ncycles || maxcycles < 0 || !(tol >= 0.0)) return fail(c, WL_EINVAL, "wl_solve: bad argument");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_solve: coefficients not set");
+    return solve_impl(c, p, b, tol, maxcycles, hist, ncycles);
+}
+
+int wl_project(wl_ctx* c, void* u, const void* L, void* p, double tol, int maxcycles, double* hist, int* ncycles) {
+    if (!c) return WL_EINVAL;
+    if (!u || !p || !hist || !ncycles || maxcycles < 0 || !(tol >= 0.0)) return fail(c, WL_EINVAL, "wl_project: bad argument");
+    int rc;
+    if (L && (rc = DISPATCH(c, set_coeff)(c, L))) return rc;
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_project: coefficients not set");
+    if (!c->b0) {
+        if (cudaMalloc(&c->b0, (size_t)c->lev[0].g.M * c->esz) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "wl_project: cudaMalloc(b)"); }
+    }
+    if ((rc = DISPATCH(c, divergence)(c, u, c->b0))) return rc;
+    int src = solve_impl(c, p, c->b0, tol, maxcycles, hist, ncycles);
+    if (src < 0) return src;
+    if ((rc = DISPATCH(c, gradient)(c, u, p))) return rc;
+    CU(c, cudaStreamSynchronize(c->stream));
+    return src;
+}
+
+int wl_project_host(wl_ctx* c, void* u_host, const void* L_host, void* p_host, double tol, int maxcycles, double* hist,
+                    int* ncycles) {
+    if (!c) return WL_EINVAL;
+    if (!u_host || !p_host || !hist || !ncycles) return fail(c, WL_EINVAL, "wl_project_host: null pointer");
+    const size_t cell_bytes = (size_t)c->lev[0].g.M * c->esz;
+    const size_t face_bytes = cell_bytes * c->n;
+    if (!c->stage_u && cudaMalloc(&c->stage_u, face_bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "cudaMalloc(stage_u)"); }
+    if (!c->stage_p && cudaMalloc(&c->stage_p, cell_bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "cudaMalloc(stage_p)"); }
+    if (L_host && !c->stage_L && cudaMalloc(&c->stage_L, face_bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "cudaMalloc(stage_L)"); }
+    CU(c, cudaMemcpyAsync(c->stage_u, u_host, face_bytes, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->stage_p, p_host, cell_bytes, cudaMemcpyHostToDevice, c->stream));
+    if (L_host) CU(c, cudaMemcpyAsync(c->stage_L, L_host, face_bytes, cudaMemcpyHostToDevice, c->stream));
+    int src = wl_project(c, c->stage_u, L_host ? c->stage_L : nullptr, c->stage_p, tol, maxcycles, hist, ncycles);
+    if (src < 0) return src;
+    CU(c, cudaMemcpyAsync(u_host, c->stage_u, face_bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaMemcpyAsync(p_host, c->stage_p, cell_bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return src;
+}
+
+int wl_divergence(wl_ctx* c, const void* u, void* b) {
+    if (!c) return WL_EINVAL;
+    if (!u || !b) return fail(c, WL_EINVAL, "wl_divergence: null pointer");
+    return DISPATCH(c, divergence)(c, u, b);
+}
+
+int wl_gradient(wl_ctx* c, void* u, const void* p) {
+    if (!c) return WL_EINVAL;
+    if (!u || !p) return fail(c, WL_EINVAL, "wl_gradient: null pointer");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_gradient: coefficients not set");
+    return DISPATCH(c, gradient)(c, u, p);
+}
+
+int wl_jacobi(wl_ctx* c, int level, void* x, const void* b, int sweeps) {
+    if (level_check(c, level, false)) return c ? fail(c, WL_EINVAL, "wl_jacobi: bad level") : WL_EINVAL;
+    if (!x || !b || sweeps < 0) return fail(c, WL_EINVAL, "wl_jacobi: bad argument");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_jacobi: coefficients not set");
+    return DISPATCH(c, jacobi)(c, level, x, b, c->lev[level].x[1], sweeps);
+}
+
+int wl_residual_restrict(wl_ctx* c, int level, const void* x, const void* b, void* bc) {
+    if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_residual_restrict: bad level") : WL_EINVAL;
+    if (!x || !b || !bc) return fail(c, WL_EINVAL, "wl_residual_restrict: null pointer");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_residual_restrict: coefficients not set");
+    return DISPATCH(c, residual_restrict)(c, level, x, b, bc, nullptr);
+}
+
+int wl_prolong_correct(wl_ctx* c, int level, const void* xc, void* x) {
+    if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_prolong_correct: bad level") : WL_EINVAL;
+    if (!x || !xc) return fail(c, WL_EINVAL, "wl_prolong_correct: null pointer");
+    return DISPATCH(c, prolong)(c, level, xc, x);
+}
+
+int wl_vcycle_level(wl_ctx* c, int level, void* x, const void* b) {
+    if (level_check(c, level, false)) return c ? fail(c, WL_EINVAL, "wl_vcycle_level: bad level") : WL_EINVAL;
+    if (!x || !b) return fail(c, WL_EINVAL, "wl_vcycle_level: null pointer");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle_level: coefficients not set");
+    return DISPATCH(c, vcycle_generic)(c, level, x, b, c->lev[level].x[1]);
+}
+
+int wl_residual_norm(wl_ctx* c, const void* p, const void* b, double* rnorm_out, double* mean_out) {
+    if (!c) return WL_EINVAL;
+    if (!p || !b || !rnorm_out) return fail(c, WL_EINVAL, "wl_residual_norm: null pointer");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_residual_norm: coefficients not set");
+    int rc = DISPATCH(c, resnorm)(c, p, b);
+    if (rc) return rc;
+    if ((rc = read_scalars(c))) return rc;
+    *rnorm_out = bits_to_double(c->h_scal->absmax_bits[1]);
+    if (mean_out) *mean_out = c->h_scal->mean_p;
+    return WL_OK;
+}
+
+int wl_num_levels(const wl_ctx* c) { return c ? c->nlev : WL_EINVAL; }
+
+int wl_level_dims(const wl_ctx* c, int level, int64_t* out) {
+    if (!c || !out || level < 0 || level >= c->nlev) return WL_EINVAL;
+    const Grid& g = c->lev[level].g;
+    out[0] = g.N0;
+    out[1] = g.N1;
+    if (c->n > 2) out[2] = g.N2;
+    return WL_OK;
+}
+
+int wl_get_coeff(const wl_ctx* c, int level, void* out) {
+    if (!c || !out || level < 0 || level >= c->nlev) return WL_EINVAL;
+    if (!c->have_coeff) return WL_ESTATE;
+    const Level& v = c->lev[level];
+    cudaError_t e = cudaMemcpyAsync(out, v.L, (size_t)v.g.M * c->n * c->esz, cudaMemcpyDeviceToDevice, c->stream);
+    return e == cudaSuccess ? WL_OK : WL_ECUDA;
+}
+
+int64_t wl_launch_count(const wl_ctx* c) { return c ? c->launches : 0; }
+
+const char* wl_last_error(const wl_ctx* c) { return c ? c->err : g_create_err; }
+
+}  // extern "C"

@@ -1,0 +1,79 @@
+// wl_common.cuh — grid descriptor, reductions, small device helpers shared by all kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace wl {
+
+// Plain-old-data grid descriptor passed by value to kernels.
+struct Grid {
+    int n;            // 2 or 3
+    int N0, N1, N2;   // N2 = 1 in 2-D
+    long long M;      // cells
+};
+
+__host__ __device__ inline long long cell_index(const Grid& g, int i0, int i1, int i2) {
+    return (long long)i0 + (long long)g.N0 * ((long long)i1 + (long long)g.N1 * (long long)i2);
+}
+
+// Device-side scalars of one context (one allocation, zeroed/reset by kernels, mirrored to pinned host memory).
+struct Scalars {
+    unsigned long long absmax_bits[4];  // slot 0: ||b||inf, 1: ||r||inf, 2..3 scratch (bit pattern of a non-negative double)
+    double sum_p;                       // sum of p (ordered second stage)
+    double mean_p;                      // sum_p / M
+    double nb;                          // ||b||inf
+    double tol;                         // stop tolerance of the running solve
+    int cycle;                          // cycles completed in the running solve
+    int done;                           // 1 once hist[cycle] <= tol * nb
+    int maxcycles;
+    int pad;
+};
+
+template <typename T> struct Omega;
+template <> struct Omega<float> { __host__ __device__ static constexpr float value() { return (float)(2.0 / 3.0); } };
+template <> struct Omega<double> { __host__ __device__ static constexpr double value() { return 2.0 / 3.0; } };
+
+// max over a warp / CTA of non-negative values, then one atomicMax on the bit pattern (exact, order-free:
+// the IEEE bit pattern of non-negative doubles is monotone in the value).
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// CTA-wide max of non-negative values; result valid in thread 0.  `red` = 32 doubles of shared memory.
+__device__ __forceinline__ double block_max(double v, double* red) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    v = warp_max(v);
+    if (lane == 0) red[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        v = (lane < nw) ? red[lane] : 0.0;
+        v = warp_max(v);
+    }
+    __syncthreads();
+    return v;
+}
+__device__ __forceinline__ double block_sum(double v, double* red) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    v = warp_sum(v);
+    if (lane == 0) red[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        v = (lane < nw) ? red[lane] : 0.0;
+        v = warp_sum(v);
+    }
+    __syncthreads();
+    return v;
+}
+
+__device__ __forceinline__ void atomic_max_nonneg(unsigned long long* slot, double v) {
+    atomicMax(slot, (unsigned long long)__double_as_longlong(v));
+}
+
+}  // namespace wl

@@ -1,0 +1,236 @@
+"""T2 — path parity of wl_vcycle / wl_solve / wl_project against the oracle on the BASELINE.json configs.
+
+Bars (BASELINE.json north_star "Numerical agreement"):
+  fp32: max|p_gpu - p_cpu| <= 1e-4 max|p_cpu| after a fixed cycle count; every per-cycle ||r||inf within 1e-3 relative;
+  fp64: 1e-10 for both.  Cycle counts to tolerance must be equal (+-1 only if the oracle's stopping residual is within
+  1e-3 relative of tol·||b||, i.e. the stop decision itself is inside the parity tolerance).
+Full sizes use the launch configuration bench.py times (fused kernels + CUDA graph = the defaults); where the oracle is
+too slow for a full solve (512^3: 17 s per V-cycle) a fixed small cycle count is compared element by element and the
+converged projection is checked by properties the oracle evaluates on the GPU's own output.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+P_TOL = {np.dtype(np.float32): 1e-4, np.dtype(np.float64): 1e-10}
+H_TOL = {np.dtype(np.float32): 1e-3, np.dtype(np.float64): 1e-10}
+
+
+@pytest.fixture(scope="module")
+def env(oracle_mod):
+    import torch
+    from paper_2304_08159_b200 import binding as wl, build, synth
+    build.build_cuda()
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return dict(torch=torch, wl=wl, oracle=oracle_mod, synth=synth)
+
+
+def _projector(env, cfg, dt, fused=1, graph=1):
+    wl = env["wl"]
+    pr = wl.Projector(cfg["dims"], dt)
+    wl.wl_set_option(pr.ctx, wl.WL_OPT_FUSED, fused)
+    wl.wl_set_option(pr.ctx, wl.WL_OPT_GRAPH, graph)
+    return pr
+
+
+def _check_hist(hist, ref, dt):
+    assert hist.shape == ref.shape, (hist.shape, ref.shape)
+    rel = np.abs(hist / ref - 1.0).max()
+    assert rel <= H_TOL[np.dtype(dt)], (rel, hist, ref)
+
+
+def _check_p(p, ref, dt):
+    err = np.abs(p.astype(np.float64) - ref.astype(np.float64)).max() / np.abs(ref).max()
+    assert err <= P_TOL[np.dtype(dt)], err
+    return err
+
+
+def _run_solve_parity(env, cfg, dt, K, fused=1, graph=1):
+    """Exactly K cycles (tol = 0) on both sides; p and history compared."""
+    torch, wl = env["torch"], env["wl"]
+    o = env["oracle"].Oracle(cfg["dims"], dt)
+    L, u = cfg["L"].astype(dt), cfg["u"].astype(dt)
+    o.set_coeff(L)
+    b = o.divergence(u)
+    p_ref, hist_ref, nc_ref, rc_ref = o.solve(np.zeros_like(b), b, 0.0, K)
+    pr = _projector(env, cfg, dt, fused, graph)
+    wl.wl_set_coeff(pr.ctx, torch.from_numpy(L).cuda())
+    bd = pr.empty_cells()
+    wl.wl_divergence(pr.ctx, torch.from_numpy(u).cuda(), bd)
+    p = pr.zeros_cells()
+    hist, nc, rc = wl.wl_solve(pr.ctx, p, bd, 0.0, K)
+    assert (nc, rc) == (nc_ref, rc_ref) == (K, wl.WL_NOT_CONVERGED)
+    _check_hist(hist, hist_ref, dt)
+    _check_p(p.cpu().numpy(), p_ref, dt)
+    assert abs(p.double().mean().item()) <= 10 * np.finfo(dt).eps * np.abs(p_ref).max()
+    pr.close()
+    return hist_ref
+
+
+@pytest.mark.parametrize("fused,graph", [(0, 0), (1, 0), (1, 1)])
+def test_config0_ten_cycles(env, fused, graph):
+    """BASELINE configs[0]: 2-D 64x64 fp32 uniform, 4 coarsenings, 10 V-cycles, p0 = 0."""
+    cfg = env["synth"].make_config(0)
+    hist = _run_solve_parity(env, cfg, np.float32, 10, fused, graph)
+    assert hist.shape == (11,)
+
+
+@pytest.mark.parametrize("config,scale,dt", [(1, 4, np.float32), (1, 4, np.float64), (2, 2, np.float32),
+                                             (2, 2, np.float64), (3, 4, np.float32), (3, 4, np.float64),
+                                             (4, 4, np.float32)])
+@pytest.mark.parametrize("fused,graph", [(0, 0), (1, 1)])
+def test_reduced_configs_fixed_cycles(env, config, scale, dt, fused, graph):
+    cfg = env["synth"].make_config(config, dtype=dt, scale=scale)
+    _run_solve_parity(env, cfg, dt, 8, fused, graph)
+
+
+def _run_to_tolerance(env, cfg, dt, fused=1, graph=1):
+    torch, wl = env["torch"], env["wl"]
+    o = env["oracle"].Oracle(cfg["dims"], dt)
+    L, u = cfg["L"].astype(dt), cfg["u"].astype(dt)
+    shape = tuple(reversed(cfg["dims"]))
+    pr = _projector(env, cfg, dt, fused, graph)
+    ud = torch.from_numpy(u).cuda()
+    Ld = torch.from_numpy(L).cuda()
+    p = pr.zeros_cells()
+    if cfg["call"] == "project":
+        u_ref, p_ref, hist_ref, nc_ref, rc_ref = o.project(u, L, np.zeros(shape, dt), cfg["tol"], cfg["maxcycles"])
+        hist, nc, rc = wl.wl_project(pr.ctx, ud, Ld, p, cfg["tol"], cfg["maxcycles"])
+    else:
+        o.set_coeff(L)
+        b = o.divergence(u)
+        p_ref, hist_ref, nc_ref, rc_ref = o.solve(np.zeros(shape, dt), b, cfg["tol"], cfg["maxcycles"])
+        wl.wl_set_coeff(pr.ctx, Ld)
+        bd = pr.empty_cells()
+        wl.wl_divergence(pr.ctx, ud, bd)
+        hist, nc, rc = wl.wl_solve(pr.ctx, p, bd, cfg["tol"], cfg["maxcycles"])
+        u_ref = None
+    if nc != nc_ref:
+        # allowed only when the stop decision is inside the parity tolerance (c-20)
+        thr = cfg["tol"] * hist_ref[0]
+        k = min(nc, nc_ref)
+        assert abs(nc - nc_ref) == 1 and abs(hist_ref[k] / thr - 1.0) <= H_TOL[np.dtype(dt)], (nc, nc_ref, hist, hist_ref)
+    else:
+        assert rc == rc_ref
+        _check_hist(hist, hist_ref, dt)
+        _check_p(p.cpu().numpy(), p_ref, dt)
+        if u_ref is not None:
+            du = np.abs(ud.cpu().numpy() - u_ref).max() / np.abs(u_ref).max()
+            assert du <= P_TOL[np.dtype(dt)], du
+    pr.close()
+    return nc, rc
+
+
+def test_config1_full_cylinder_to_tolerance(env):
+    """BASELINE configs[1]: 2-D 1024x1024 fp32 cylinder, solve to 1e-4 (expected to end at the 32-cycle cap; c-19)."""
+    cfg = env["synth"].make_config(1)
+    nc, rc = _run_to_tolerance(env, cfg, np.float32)
+    assert nc >= 20
+
+
+def test_config2_full_sphere_project(env):
+    """BASELINE configs[2]: 3-D 128^3 fp32 sphere, full wl_project."""
+    cfg = env["synth"].make_config(2)
+    nc, rc = _run_to_tolerance(env, cfg, np.float32)
+    assert rc == 0 and 10 <= nc <= 32
+
+
+@pytest.mark.parametrize("dt,K", [(np.float32, 3), (np.float64, 2)])
+def test_config3_full_256_fixed_cycles(env, dt, K):
+    """BASELINE configs[3]: 3-D 256^3 uniform L, Taylor-Green + noise, fp32 and fp64 (6 coarsenings)."""
+    cfg = env["synth"].make_config(3, dtype=dt)
+    _run_solve_parity(env, cfg, dt, K)
+
+
+def test_config3_half_size_to_tolerance_fp64(env):
+    cfg = env["synth"].make_config(3, dtype=np.float64, scale=2)
+    nc, rc = _run_to_tolerance(env, cfg, np.float64)
+    assert rc == 0
+
+
+def test_config4_full_512_properties_and_two_cycles(env):
+    """BASELINE configs[4]: 3-D 512^3 fp32, 32 spheres, wl_project to tolerance — bench.py's workload and launch
+    configuration.  The oracle needs 17 s per V-cycle here, so: (a) two V-cycles compared element by element;
+    (b) the converged projection checked by what the ORACLE computes from the GPU's own p and u:
+    hist[-1] = ||b - A p||inf, div(u_out) = b - A p, u_out = u - L grad p, mean(p) = 0, monotone history."""
+    torch, wl = env["torch"], env["wl"]
+    dt = np.float32
+    cfg = env["synth"].make_config(4)
+    L, u = cfg["L"], cfg["u"]
+    o = env["oracle"].Oracle(cfg["dims"], dt)
+    o.set_coeff(L)
+    b = o.divergence(u)
+    pr = _projector(env, cfg, dt)
+    Ld = torch.from_numpy(L).cuda()
+    ud = torch.from_numpy(u).cuda()
+    wl.wl_set_coeff(pr.ctx, Ld)
+    bd = pr.empty_cells()
+    wl.wl_divergence(pr.ctx, ud, bd)
+    assert np.abs(bd.cpu().numpy() - b).max() <= 1e-6
+    # (a) two cycles
+    p = pr.zeros_cells()
+    p_ref = np.zeros_like(b)
+    for k in range(2):
+        nrm = wl.wl_vcycle(pr.ctx, p, bd)
+        p_ref, nrm_ref = o.vcycle(p_ref, b)
+        assert abs(nrm / nrm_ref - 1.0) <= 1e-3
+    _check_p(p.cpu().numpy(), p_ref, dt)
+    del p_ref
+    # (b) full projection
+    p.zero_()
+    hist, nc, rc = wl.wl_project(pr.ctx, ud, None, p, cfg["tol"], cfg["maxcycles"])
+    assert rc == 0 and 10 <= nc <= 32
+    assert np.all(np.diff(hist) < 0)
+    assert hist[0] == np.abs(b).max()
+    assert hist[-1] <= cfg["tol"] * hist[0] < hist[-2]
+    pg = p.cpu().numpy()
+    r, nrm = o.residual(pg, b)
+    assert abs(hist[-1] / nrm - 1.0) <= 1e-3
+    assert abs(pg.astype(np.float64).mean()) <= 1e-6 * np.abs(pg).max()
+    ug = ud.cpu().numpy()
+    u_exp = o.gradient_correct(u, pg)
+    assert np.abs(ug - u_exp).max() <= 1e-6 * max(1.0, np.abs(u_exp).max())
+    div_after = o.divergence(ug)
+    assert np.abs(div_after).max() <= 1.1e-4 * hist[0]
+    assert np.abs(div_after - r).max() <= 2e-5 * hist[0]
+    pr.close()
+
+
+def test_warm_start_and_repeat_calls(env):
+    """Projecting the already-corrected field starts from a divergence that is the first call's final residual; solving
+    again from the solution runs zero cycles and leaves p unchanged up to its (already zero) mean."""
+    torch, wl = env["torch"], env["wl"]
+    cfg = env["synth"].make_config(2, scale=4)
+    pr = _projector(env, cfg, np.float32)
+    ud = torch.from_numpy(cfg["u"]).cuda()
+    bd = pr.empty_cells()
+    wl.wl_divergence(pr.ctx, ud, bd)
+    p = pr.zeros_cells()
+    hist, nc, rc = wl.wl_project(pr.ctx, ud, torch.from_numpy(cfg["L"]).cuda(), p, 1e-4, 32)
+    assert rc == 0 and nc > 5
+    b2 = pr.empty_cells()
+    wl.wl_divergence(pr.ctx, ud, b2)
+    assert abs(b2.abs().max().item() / hist[-1] - 1.0) <= 1e-3   # div(u_out) = b - A p
+    p_before = p.clone()
+    hist2, nc2, rc2 = wl.wl_solve(pr.ctx, p, bd, 1e-4, 32)
+    assert nc2 == 0 and rc2 == 0 and hist2.shape == (1,) and abs(hist2[0] / hist[-1] - 1.0) <= 1e-3
+    assert (p - p_before).abs().max().item() <= 1e-6 * p_before.abs().max().item()
+    pr.close()
+
+
+def test_project_host_matches_device_call(env):
+    torch, wl = env["torch"], env["wl"]
+    cfg = env["synth"].make_config(2, scale=4)
+    pr = _projector(env, cfg, np.float32)
+    ud = torch.from_numpy(cfg["u"]).cuda()
+    Ld = torch.from_numpy(cfg["L"]).cuda()
+    p = pr.zeros_cells()
+    hist, nc, rc = wl.wl_project(pr.ctx, ud, Ld, p, 1e-4, 32)
+    uh = torch.from_numpy(cfg["u"].copy()).pin_memory()
+    Lh = torch.from_numpy(cfg["L"].copy()).pin_memory()
+    ph = torch.zeros(pr.cell_shape(), dtype=torch.float32).pin_memory()
+    hist_h, nc_h, rc_h = wl.wl_project_host(pr.ctx, uh, Lh, ph, 1e-4, 32)
+    assert nc_h == nc and rc_h == rc and np.array_equal(hist_h, hist)
+    assert torch.equal(uh, ud.cpu()) and torch.equal(ph, p.cpu())
+    pr.close()
