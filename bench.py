@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py — the pressure projection on seeded synthetic grids, timed on the B200 (driver contract: see DESIGN.md §8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+One "step" = one pass of the whole hot path (SURVEY.md §8(a) H0–H9): ``wl_project(u, L, p=0)`` — coefficient hierarchy,
+divergence, GMG V-cycles to ||r||inf <= 1e-4 ||b||inf (cap 32), pressure-gradient correction — on BASELINE.json
+``configs[C]`` (default C = 4: 3-D 512^3 fp32, 32 seeded spheres, the largest single-GPU configuration).
+
+The JSON line (rank 0):
+  value      fine cells/s per V-cycle through the whole projection = n_gpus * M * cycles / seconds per step,
+             inputs resident in HBM when the timed region starts (CUDA events on the ctx stream, summed over K steps);
+  e2e        the same metric through ``wl_project_host`` with pinned HOST buffers: H2D of u, L, p and D2H of u, p inside
+             the timed region;
+  roofline   the dominant kernel (the fused level-0 DOWN kernel: 2 pre-sweeps + residual + restriction) timed alone with
+             CUDA events through ``wl_down``; achieved = algorithmic bytes (read p, b, n·L, write p, write
+             b_c = (n+3+1/2^n)·s per cell) / duration, against MEASURED_PEAKS.json ``hbm_gbs``;
+  cpu_baseline  the oracle as it stands on the box's host cores (1 thread), on a bounded sample (one V-cycle of the same
+             workload);
+  extra keys: ms per projection, ms per V-cycle (graph launches alone), effective GB/s per V-cycle (56 B/cell model).
+
+N > 1 (torchrun): "replicas only" — every rank projects its own copy of the grid, no collective on the data path
+(BASELINE.json north_star: one GPU, no sharding); value = units all ranks processed / max-over-ranks time.
+``--impl reference`` times the CPU oracle (rank 0 only) on the same config and metric.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "GMG V-cycle fine cells/s (whole projection)"
+UNIT = "cells/s"
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _loop(self):
+        nv = self._nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        med = int(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def _algorithmic_bytes_down(n: int, esz: int) -> float:
+    """Level-0 DOWN kernel, per cell: read p, b, n·L; write p; write b_c (1/2^n of a cell)."""
+    return (n + 3 + 1.0 / 2 ** n) * esz
+
+
+def run_reference(args, rank: int):
+    """The oracle timed on host cores: each step = one V-cycle (+ mean removal + residual norm) of the same workload."""
+    if rank != 0:
+        return
+    from paper_2304_08159_b200 import synth
+    import oracle
+    oracle.build()
+    cfg = synth.make_config(args.config, scale=args.scale)
+    dims, dt = cfg["dims"], cfg["dtype"]
+    M = int(np.prod(dims))
+    o = oracle.Oracle(dims, dt)
+    o.set_coeff(cfg["L"])
+    b = o.divergence(cfg["u"])
+    p = np.zeros(tuple(reversed(dims)), dt)
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        p, _ = o.vcycle(p, b)
+        t1 = time.perf_counter()
+        if it >= args.warmup:
+            times.append(t1 - t0)
+    sec = float(np.sum(times)) / max(1, len(times))
+    val = M / sec
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if dt == np.float32 else "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "dims": list(dims), "sample": "each step = one oracle V-cycle"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"{args.steps} V-cycles of {cfg['name']} after {args.warmup} warm-up cycles"},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--scale", type=int, default=1, help="divide every extent (debug only; the default 1 is the workload)")
+    ap.add_argument("--dtype", default=None, choices=[None, "float32", "float64"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--fused", type=int, default=1)
+    ap.add_argument("--graph", type=int, default=1)
+    ap.add_argument("--kernel-reps", type=int, default=20)
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if args.warmup < 3:
+        args.warmup = 3  # timing rule: W >= 3
+
+    import torch
+    import torch.distributed as dist
+    from paper_2304_08159_b200 import binding as wl, synth, build
+    build.build_cuda()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (there is no CPU path)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    dt_np = None if args.dtype is None else np.dtype(args.dtype)
+    cfg = synth.make_config(args.config, dtype=dt_np, scale=args.scale)
+    dims, dt = cfg["dims"], cfg["dtype"]
+    n, M, esz = len(dims), int(np.prod(dims)), cfg["dtype"].itemsize
+    tol, maxc = cfg["tol"], cfg["maxcycles"]
+    if tol == 0.0:  # config 0 is a fixed-cycle case
+        tol = 0.0
+
+    pr = wl.Projector(dims, dt, dev)
+    wl.wl_set_option(pr.ctx, wl.WL_OPT_FUSED, args.fused)
+    wl.wl_set_option(pr.ctx, wl.WL_OPT_GRAPH, args.graph)
+    u_host = torch.from_numpy(cfg["u"]).pin_memory()
+    L_host = torch.from_numpy(cfg["L"]).pin_memory()
+    u0 = u_host.to(dev, non_blocking=True)
+    Ld = L_host.to(dev, non_blocking=True)
+    u = torch.empty_like(u0)
+    p = pr.zeros_cells()
+    stream = torch.cuda.current_stream()
+
+    def one_step():
+        u.copy_(u0)
+        p.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        hist, nc, rc = wl.wl_project(pr.ctx, u, Ld, p, tol, maxc)
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1), hist, nc, rc
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    launches0 = wl.wl_launch_count(pr.ctx)
+    ms = []
+    with ClockSampler(local_rank) as clk:
+        for _ in range(args.steps):
+            t, hist, nc, rc = one_step()
+            ms.append(t)
+        launches = wl.wl_launch_count(pr.ctx) - launches0
+        barrier()
+        total_ms = float(np.sum(ms))
+
+        # e2e: same projection through the host-buffer entry point (H2D u, L, p; D2H u, p inside the timed region)
+        if not args.no_e2e:
+            uh = torch.empty_like(u_host).pin_memory()
+            ph = torch.zeros(pr.cell_shape(), dtype=pr.torch_dtype).pin_memory()
+            e2e_ms = []
+            for it in range(2 + args.steps):
+                uh.copy_(u_host)
+                ph.zero_()
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                h2, nc2, rc2 = wl.wl_project_host(pr.ctx, uh, L_host, ph, tol, maxc)
+                e1.record(stream)
+                e1.synchronize()
+                if it >= 2:
+                    e2e_ms.append(e0.elapsed_time(e1))
+            e2e_total = float(np.sum(e2e_ms))
+
+        # V-cycle alone (graph launches back to back, no readback) and the dominant kernels alone
+        bd = pr.empty_cells()
+        wl.wl_divergence(pr.ctx, u0, bd)
+        p.zero_()
+        for _ in range(3):
+            wl.wl_vcycle(pr.ctx, p, bd, want_norm=False)
+        reps = max(5, args.kernel_reps)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(reps):
+            wl.wl_vcycle(pr.ctx, p, bd, want_norm=False)
+        e1.record(stream)
+        e1.synchronize()
+        vcycle_ms = e0.elapsed_time(e1) / reps
+
+        kern = {}
+        if pr.num_levels > 1:
+            xo = pr.empty_cells()
+            for name, fn in (("down", lambda: wl.wl_down(pr.ctx, 0, p, bd, xo)),
+                             ("up", lambda: wl.wl_up(pr.ctx, 0, xo, None, bd, p))):
+                for _ in range(3):
+                    fn()
+                l0 = wl.wl_launch_count(pr.ctx)
+                torch.cuda.synchronize()
+                e0.record(stream)
+                for _ in range(reps):
+                    fn()
+                e1.record(stream)
+                e1.synchronize()
+                kern[name] = {"ms": e0.elapsed_time(e1) / reps, "launches_per_call": (wl.wl_launch_count(pr.ctx) - l0) // reps}
+    clocks = clk.summary()
+
+    # max over ranks
+    if world > 1:
+        t = torch.tensor([total_ms, 0.0 if args.no_e2e else e2e_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t[0].item())
+        if not args.no_e2e:
+            e2e_total = float(t[1].item())
+
+    sec_per_step = total_ms / 1e3 / args.steps
+    value = world * M * nc / sec_per_step if nc > 0 else 0.0
+    peak, peak_src = _peaks()
+    roof = None
+    if kern:
+        bytes_down = _algorithmic_bytes_down(n, esz) * M
+        ach = bytes_down / (kern["down"]["ms"] * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "level-0 DOWN (2 pre-sweeps + residual + restriction), via wl_down",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_down,
+                "launches_per_call": kern["down"]["launches_per_call"], "ms": kern["down"]["ms"],
+                "up_kernel": {"ms": kern["up"]["ms"], "achieved": bytes_down / (kern["up"]["ms"] * 1e-3) / 1e9,
+                              "launches_per_call": kern["up"]["launches_per_call"]}}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if dt == np.float32 else "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "dims": list(dims), "cells": M, "tol": tol, "maxcycles": maxc,
+                   "cycles_run": int(nc), "converged": bool(rc == 0), "fused": args.fused, "graph": args.graph,
+                   "l2": "inputs larger than L2 (no flush needed)" if (n + 3) * M * esz > 200e6 else "working set fits L2",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "ms_per_projection": sec_per_step * 1e3,
+        "vcycle": {"ms": vcycle_ms, "cells_per_s": M / (vcycle_ms * 1e-3),
+                   "effective_GBps_56B_model": (2 * (n + 3) + 2.0 / 2 ** n) * esz * (2 ** n / (2 ** n - 1.0)) * M / (vcycle_ms * 1e-3) / 1e9},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": roof,
+    }
+    if not args.no_e2e:
+        e2e_sec = e2e_total / 1e3 / args.steps
+        h2d = u_host.numel() * esz + L_host.numel() * esz + M * esz
+        d2h = u_host.numel() * esz + M * esz
+        line["e2e"] = {"value": world * M * nc2 / e2e_sec, "unit": UNIT, "ms_per_step": e2e_sec * 1e3,
+                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        # the oracle as it stands, one thread, bounded sample: one V-cycle of the same workload
+        import oracle
+        oracle.build()
+        o = oracle.Oracle(dims, dt)
+        o.set_coeff(cfg["L"])
+        bo = o.divergence(cfg["u"])
+        po = np.zeros(tuple(reversed(dims)), dt)
+        ncyc = 1 if M >= (1 << 26) else max(1, min(10, int(2e8 // M)))
+        t0 = time.perf_counter()
+        for _ in range(ncyc):
+            po, _ = o.vcycle(po, bo)
+        tc = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": M * ncyc / tc, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{ncyc} oracle V-cycle(s) of {cfg['name']} ({tc:.1f} s), host nproc={os.cpu_count()}"}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    pr.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -38,6 +38,8 @@ SIGNATURES = {
     "wl_jacobi": (_i32, [_vp, _i32, _vp, _vp, _i32]),
     "wl_residual_restrict": (_i32, [_vp, _i32, _vp, _vp, _vp]),
     "wl_prolong_correct": (_i32, [_vp, _i32, _vp, _vp]),
+    "wl_down": (_i32, [_vp, _i32, _vp, _vp, _vp, _vp]),
+    "wl_up": (_i32, [_vp, _i32, _vp, _vp, _vp, _vp]),
     "wl_vcycle_level": (_i32, [_vp, _i32, _vp, _vp]),
     "wl_residual_norm": (_i32, [_vp, _vp, _vp, _f64p, _f64p]),
     "wl_num_levels": (_i32, [_vp]),
@@ -190,6 +192,16 @@ def wl_residual_restrict(ctx, level: int, x, b, bc):
 
 def wl_prolong_correct(ctx, level: int, xc, x):
     return _check(ctx, load().wl_prolong_correct(ctx, int(level), _dptr(xc), _dptr(x)), "wl_prolong_correct")
+
+
+def wl_down(ctx, level: int, x_in, b, x_out, bc=None):
+    """x_out = J(J(x_in)) (x_in=None: from zero); bc (None: the context's level+1 rhs) = R(b - A x_out)."""
+    return _check(ctx, load().wl_down(ctx, int(level), _dptr(x_in), _dptr(b), _dptr(x_out), _dptr(bc)), "wl_down")
+
+
+def wl_up(ctx, level: int, x_in, xc, b, x_out):
+    """x_out = J(J(x_in + P xc)); xc=None: the context's level+1 iterate."""
+    return _check(ctx, load().wl_up(ctx, int(level), _dptr(x_in), _dptr(xc), _dptr(b), _dptr(x_out)), "wl_up")
 
 
 def wl_vcycle_level(ctx, level: int, x, b):

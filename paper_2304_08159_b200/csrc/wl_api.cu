@@ -26,6 +26,7 @@ struct Level {
     void* L = nullptr;      // n*M coefficients (ctx-owned copy / coarsened)
     void* x[2] = {nullptr, nullptr};  // level >= 1: iterate ping-pong; level 0: x[1] = ctx-owned scratch only
     void* b = nullptr;      // level >= 1: restricted residual
+    void* tmp = nullptr;    // generic path only: second half of the Jacobi ping-pong (allocated on first use)
 };
 
 thread_local char g_create_err[256] = "";
@@ -143,6 +144,42 @@ struct Impl {
         k_prolong_add<T, ND><<<grid_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, k.g, P(xc), P(x));
         KCHECK(c, "k_prolong_add");
         return WL_OK;
+    }
+
+    static int ensure_tmp(wl_ctx* c, int l) {
+        Level& v = c->lev[l];
+        if (!v.tmp && cudaMalloc(&v.tmp, (size_t)v.g.M * sizeof(T)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(c, WL_ENOMEM, "cudaMalloc(level tmp)");
+        }
+        return WL_OK;
+    }
+
+    // DOWN half of level l with generic kernels: x_out = J(J(x_in)) (x_in == nullptr: from zero), bc = R(b - A x_out).
+    static int down_generic(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out, void* bc) {
+        int rc;
+        Level& v = c->lev[l];
+        if ((rc = ensure_tmp(c, l))) return rc;
+        if (x_in) {
+            if ((rc = jacobi_sweep(c, l, x_in, b, v.tmp))) return rc;
+        } else {
+            k_jacobi_from_zero<T, ND><<<grid_for(c, v.g.M), kBlock, 0, c->stream>>>(v.g, P(v.L), P(b), P(v.tmp));
+            KCHECK(c, "k_jacobi_from_zero");
+        }
+        if ((rc = jacobi_sweep(c, l, v.tmp, b, x_out))) return rc;
+        return residual_restrict(c, l, x_out, b, bc, nullptr);
+    }
+
+    // UP half of level l with generic kernels: x_out = J(J(x_in + P xc)).
+    static int up_generic(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out) {
+        int rc;
+        Level& f = c->lev[l];
+        Level& k = c->lev[l + 1];
+        if ((rc = ensure_tmp(c, l))) return rc;
+        k_prolong_out<T, ND><<<grid_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, k.g, P(xc), P(x_in), P(x_out));
+        KCHECK(c, "k_prolong_out");
+        if ((rc = jacobi_sweep(c, l, x_out, b, f.tmp))) return rc;
+        return jacobi_sweep(c, l, f.tmp, b, x_out);
     }
 
     // VCYCLE(l) with generic kernels.  x, b: arrays of level l; tmp: scratch of level l.
@@ -379,6 +416,7 @@ void wl_destroy(wl_ctx* c) {
         if (v.x[0]) cudaFree(v.x[0]);
         if (v.x[1]) cudaFree(v.x[1]);
         if (v.b) cudaFree(v.b);
+        if (v.tmp) cudaFree(v.tmp);
     }
     if (c->d_scal) cudaFree(c->d_scal);
     if (c->d_partials) cudaFree(c->d_partials);
@@ -503,6 +541,20 @@ int wl_prolong_correct(wl_ctx* c, int level, const void* xc, void* x) {
     if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_prolong_correct: bad level") : WL_EINVAL;
     if (!x || !xc) return fail(c, WL_EINVAL, "wl_prolong_correct: null pointer");
     return DISPATCH(c, prolong)(c, level, xc, x);
+}
+
+int wl_down(wl_ctx* c, int level, const void* x_in, const void* b, void* x_out, void* bc) {
+    if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_down: bad level") : WL_EINVAL;
+    if (!b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_down: bad pointer");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_down: coefficients not set");
+    return DISPATCH(c, down_generic)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
+}
+
+int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b, void* x_out) {
+    if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_up: bad level") : WL_EINVAL;
+    if (!x_in || !b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_up: bad pointer");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_up: coefficients not set");
+    return DISPATCH(c, up_generic)(c, level, x_in, xc ? xc : c->lev[level + 1].x[0], b, x_out);
 }
 
 int wl_vcycle_level(wl_ctx* c, int level, void* x, const void* b) {

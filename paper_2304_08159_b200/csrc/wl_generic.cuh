@@ -212,6 +212,16 @@ __global__ void k_prolong_add(Grid gf, Grid gc, const T* __restrict__ xc, T* __r
     }
 }
 
+// H6 (first half), out of place: xout[I] = xin[I] + xc[floor(I/2)].
+template <typename T, int ND>
+__global__ void k_prolong_out(Grid gf, Grid gc, const T* __restrict__ xc, const T* __restrict__ xin, T* __restrict__ xout) {
+    for (long long I = (long long)blockIdx.x * blockDim.x + threadIdx.x; I < gf.M; I += (long long)gridDim.x * blockDim.x) {
+        int i0, i1, i2;
+        decompose<T, ND>(gf, I, i0, i1, i2);
+        xout[I] = xin[I] + xc[cell_index(gc, i0 >> 1, i1 >> 1, i2 >> 1)];
+    }
+}
+
 // ||v||inf into scal->absmax_bits[slot] (slot must have been zeroed).
 template <typename T>
 __global__ void k_absmax(long long M, const T* __restrict__ v, Scalars* scal, int slot) {
