@@ -12,6 +12,7 @@
 #include "../../include/wl.h"
 #include "wl_common.cuh"
 #include "wl_generic.cuh"
+#include "wl_fused3d.cuh"
 
 using namespace wl;
 
@@ -51,6 +52,7 @@ struct wl_ctx {
     bool have_coeff = false;
     int opt_fused = 1, opt_graph = 1, opt_coarse_cta = 1;
     int num_sms = 148;
+    int fused_grid = 0;          // CTAs of the last fused launch (= number of sum partials it wrote)
     int64_t launches = 0;
     char err[256] = "";
 };
@@ -182,34 +184,126 @@ struct Impl {
         return jacobi_sweep(c, l, f.tmp, b, x_out);
     }
 
-    // VCYCLE(l) with generic kernels.  x, b: arrays of level l; tmp: scratch of level l.
-    static int vcycle_generic(wl_ctx* c, int l, void* x, const void* b, void* tmp) {
-        int rc;
-        Level& v = c->lev[l];
-        if (l == c->nlev - 1) {
-            int sweeps = 64;
-            if (c->nlev > 1) {
-                // x = 0 then one sweep == the closed form of the first sweep; 63 more follow
-                k_jacobi_from_zero<T, ND><<<grid_for(c, v.g.M), kBlock, 0, c->stream>>>(v.g, P(v.L), P(b), P(tmp));
-                KCHECK(c, "k_jacobi_from_zero");
-                // 63 sweeps starting from tmp, ending in x (odd count: tmp -> x -> tmp ... -> x)
-                void* cur = tmp;
-                void* oth = x;
-                for (int s = 1; s < sweeps; ++s) {
-                    if ((rc = jacobi_sweep(c, l, cur, b, oth))) return rc;
-                    void* t = cur; cur = oth; oth = t;
-                }
-                if (cur != x) CU(c, cudaMemcpyAsync(x, cur, (size_t)v.g.M * sizeof(T), cudaMemcpyDeviceToDevice, c->stream));
-                return WL_OK;
+
+    // ---- fused level halves (wl_fused3d.cuh) ---------------------------------------------------------------------
+    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = 16, FPF = 3;
+
+    // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
+    // vectors; opt_fused == 1 keeps levels smaller than one tile on the generic kernels, 2 forces them (tests).
+    static bool fused_ok(const wl_ctx* c, int l) {
+        if (ND != 3 || !c->opt_fused || l + 1 >= c->nlev) return false;
+        const Grid& g = c->lev[l].g;
+        constexpr int VEC = 16 / (int)sizeof(T);
+        if (g.N0 % (2 * VEC)) return false;
+        if (c->opt_fused == 1 && (g.N0 < FTX || g.N1 < FTY || g.N2 < 8)) return false;
+        return get_encode_tiled() != nullptr;
+    }
+
+    static bool map_cells(CUtensorMap* m, const void* base, const Grid& g, bool coarse_box) {
+        using G = F3<T, FTX, FTY>;
+        if (((uintptr_t)base & 15) != 0) return false;
+        const uint64_t d[3] = {(uint64_t)g.N0, (uint64_t)g.N1, (uint64_t)g.N2};
+        const uint32_t b[3] = {(uint32_t)(coarse_box ? G::CWX : G::WX), (uint32_t)(coarse_box ? G::CWY : G::WY), 1u};
+        return encode_map(m, base, (int)sizeof(T), 3, d, b);
+    }
+
+    template <bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS>
+    static int launch_fused(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out, void* bc) {
+        if constexpr (ND == 3) {
+            using G = F3<T, FTX, FTY>;
+            Level& f = c->lev[l];
+            CUtensorMap mx, mb, mL0, mL1, mL2, mxc;
+            bool ok = map_cells(&mb, b, f.g, false);
+            ok = ok && map_cells(&mL0, P(f.L), f.g, false) && map_cells(&mL1, P(f.L) + f.g.M, f.g, false) &&
+                 map_cells(&mL2, P(f.L) + 2 * f.g.M, f.g, false);
+            if (ZERO_IN) mx = mb; else ok = ok && map_cells(&mx, x_in, f.g, false);
+            if (PROLONG) ok = ok && map_cells(&mxc, xc, c->lev[l + 1].g, true); else mxc = mb;
+            if (!ok) return fail(c, WL_ECUDA, "cuTensorMapEncodeTiled refused a level array (alignment?)");
+            Fused3Params<T> prm;
+            prm.N0 = f.g.N0; prm.N1 = f.g.N1; prm.N2 = f.g.N2;
+            prm.tiles_x = (f.g.N0 + FTX - 1) / FTX;
+            prm.tiles_y = (f.g.N1 + FTY - 1) / FTY;
+            prm.steps = (long long)prm.tiles_x * prm.tiles_y * f.g.N2;
+            prm.xout = P(x_out);
+            prm.bc = P(bc);
+            prm.scal = c->d_scal;
+            prm.partials = c->d_partials;
+            auto kern = k_fused3d<T, FTX, FTY, FPF, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS>;
+            constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF, PROLONG>();
+            static bool attr_set = false;
+            if (!attr_set) {
+                CU(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                attr_set = true;
             }
-            return jacobi(c, l, x, b, tmp, sweeps);
+            long long g = prm.steps / 8;
+            if (g < 1) g = 1;
+            if (g > c->num_sms) g = c->num_sms;
+            if (NORMS && g > kMaxPartials) g = kMaxPartials;
+            c->fused_grid = (int)g;
+            kern<<<(int)g, G::NT, smem, c->stream>>>(mx, mb, mL0, mL1, mL2, mxc, prm);
+            KCHECK(c, "k_fused3d");
+            return WL_OK;
+        } else {
+            return fail(c, WL_EINVAL, "fused kernels are 3-D only");
+        }
+    }
+
+    // DOWN half of level l: x_out = J(J(x_in)) (x_in == nullptr: from zero), bc = R(b - A x_out).
+    static int down(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out, void* bc) {
+        if (!fused_ok(c, l)) return down_generic(c, l, x_in, b, x_out, bc);
+        if (x_in) return launch_fused<false, false, false, true, true, false>(c, l, x_in, nullptr, b, x_out, bc);
+        return launch_fused<false, true, false, true, true, false>(c, l, nullptr, nullptr, b, x_out, bc);
+    }
+
+    // UP half of level l: x_out = J(J(x_in + P xc)); `norms` (level 0): also ||b - A x_out||inf -> slot 1, sum -> mean.
+    static int up(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out, bool norms) {
+        if (!fused_ok(c, l)) {
+            int rc = up_generic(c, l, x_in, xc, b, x_out);
+            if (rc || !norms) return rc;
+            return resnorm(c, x_out, b);
+        }
+        if (!norms) return launch_fused<true, false, false, false, false, false>(c, l, x_in, xc, b, x_out, nullptr);
+        k_zero_slot<<<1, 32, 0, c->stream>>>(c->d_scal, 1);
+        KCHECK(c, "k_zero_slot");
+        int rc = launch_fused<true, false, false, true, false, true>(c, l, x_in, xc, b, x_out, nullptr);
+        if (rc) return rc;
+        k_finish_mean<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_partials, c->fused_grid, c->lev[0].g.M);
+        KCHECK(c, "k_finish_mean");
+        return WL_OK;
+    }
+
+    // 64 sweeps on the coarsest level.  x_in == nullptr: from zero (correction level), result in x_out; the other
+    // buffer `x_mid` is the second half of the ping-pong.  x_in != nullptr (a one-level hierarchy): x_in may be x_out.
+    static int coarsest(wl_ctx* c, int l, const void* x_in, const void* b, void* x_mid, void* x_out) {
+        Level& v = c->lev[l];
+        int rc;
+        if (!x_in) {
+            k_jacobi_from_zero<T, ND><<<grid_for(c, v.g.M), kBlock, 0, c->stream>>>(v.g, P(v.L), P(b), P(x_mid));
+            KCHECK(c, "k_jacobi_from_zero");
+            void* cur = x_mid;
+            void* oth = x_out;
+            for (int s = 1; s < 64; ++s) {  // 63 more: x_mid -> x_out -> ... -> x_out
+                if ((rc = jacobi_sweep(c, l, cur, b, oth))) return rc;
+                void* t2 = cur; cur = oth; oth = t2;
+            }
+            return WL_OK;
+        }
+        if (x_in != x_out) CU(c, cudaMemcpyAsync(x_out, x_in, (size_t)v.g.M * sizeof(T), cudaMemcpyDeviceToDevice, c->stream));
+        return jacobi(c, l, x_out, b, x_mid, 64);
+    }
+
+    // VCYCLE(l): x_out = cycle(x_in) on level l; x_mid = level-sized scratch (may not alias x_in / x_out).
+    // x_in == nullptr means a zero initial guess (every correction level).  norms: level-0 reductions after the UP half.
+    static int vcycle(wl_ctx* c, int l, const void* x_in, const void* b, void* x_mid, void* x_out, bool norms) {
+        int rc;
+        if (l == c->nlev - 1) {
+            if ((rc = coarsest(c, l, (c->nlev > 1 && l > 0) ? nullptr : x_in, b, x_mid, x_out))) return rc;
+            return norms ? resnorm(c, x_out, b) : WL_OK;
         }
         Level& k = c->lev[l + 1];
-        if ((rc = jacobi(c, l, x, b, tmp, 2))) return rc;
-        if ((rc = residual_restrict(c, l, x, b, k.b, k.x[0]))) return rc;  // also x_{l+1} = 0
-        if ((rc = vcycle_generic(c, l + 1, k.x[0], k.b, k.x[1]))) return rc;
-        if ((rc = prolong(c, l, k.x[0], x))) return rc;
-        return jacobi(c, l, x, b, tmp, 2);
+        if ((rc = down(c, l, x_in, b, x_mid, k.b))) return rc;
+        if ((rc = vcycle(c, l + 1, nullptr, k.b, k.x[0], k.x[1], false))) return rc;
+        return up(c, l, x_mid, k.x[1], b, x_out, norms);
     }
 
     // Σp -> mean (ordered), p -= mean.
@@ -247,12 +341,15 @@ struct Impl {
         return WL_OK;
     }
 
-    // One V-cycle + mean removal + residual norm (slot 1).
+    // One V-cycle; ||b - A p||inf (slot 1) and mean(p) come out of the level-0 UP half; then p -= mean.  The norm is
+    // taken before the shift: A·1 = 0, so it differs from the oracle's (after the shift) by rounding only.
     static int cycle(wl_ctx* c, void* p, const void* b) {
         int rc;
-        if ((rc = vcycle_generic(c, 0, p, b, c->lev[0].x[1]))) return rc;
-        if ((rc = remove_mean(c, p))) return rc;
-        return resnorm(c, p, b);
+        if ((rc = vcycle(c, 0, p, b, c->lev[0].x[1], p, true))) return rc;
+        const long long M = c->lev[0].g.M;
+        k_shift<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, P(p), c->d_scal);
+        KCHECK(c, "k_shift");
+        return WL_OK;
     }
 
     static int divergence(wl_ctx* c, const void* u, void* b) {
@@ -440,7 +537,7 @@ int wl_set_stream(wl_ctx* c, void* s) {
 int wl_set_option(wl_ctx* c, int key, int value) {
     if (!c) return WL_EINVAL;
     switch (key) {
-        case WL_OPT_FUSED: c->opt_fused = value ? 1 : 0; return WL_OK;
+        case WL_OPT_FUSED: c->opt_fused = (value < 0 || value > 2) ? 1 : value; return WL_OK;
         case WL_OPT_GRAPH: c->opt_graph = value ? 1 : 0; return WL_OK;
         case WL_OPT_COARSE_CTA: c->opt_coarse_cta = value ? 1 : 0; return WL_OK;
         default: return fail(c, WL_EINVAL, "wl_set_option: unknown key");
@@ -547,21 +644,21 @@ int wl_down(wl_ctx* c, int level, const void* x_in, const void* b, void* x_out, 
     if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_down: bad level") : WL_EINVAL;
     if (!b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_down: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_down: coefficients not set");
-    return DISPATCH(c, down_generic)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
+    return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
 }
 
 int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b, void* x_out) {
     if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_up: bad level") : WL_EINVAL;
     if (!x_in || !b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_up: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_up: coefficients not set");
-    return DISPATCH(c, up_generic)(c, level, x_in, xc ? xc : c->lev[level + 1].x[0], b, x_out);
+    return DISPATCH(c, up)(c, level, x_in, xc ? xc : c->lev[level + 1].x[1], b, x_out, false);
 }
 
 int wl_vcycle_level(wl_ctx* c, int level, void* x, const void* b) {
     if (level_check(c, level, false)) return c ? fail(c, WL_EINVAL, "wl_vcycle_level: bad level") : WL_EINVAL;
     if (!x || !b) return fail(c, WL_EINVAL, "wl_vcycle_level: null pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle_level: coefficients not set");
-    return DISPATCH(c, vcycle_generic)(c, level, x, b, c->lev[level].x[1]);
+    return DISPATCH(c, vcycle)(c, level, x, b, level == 0 ? c->lev[0].x[1] : c->lev[level].x[0], x, false);
 }
 
 int wl_residual_norm(wl_ctx* c, const void* p, const void* b, double* rnorm_out, double* mean_out) {

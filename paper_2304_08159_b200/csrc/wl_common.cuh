@@ -21,6 +21,7 @@ struct Scalars {
     unsigned long long absmax_bits[4];  // slot 0: ||b||inf, 1: ||r||inf, 2..3 scratch (bit pattern of a non-negative double)
     double sum_p;                       // sum of p (ordered second stage)
     double mean_p;                      // sum_p / M
+    double shift;                       // deferred mean removal: what the next level-0 DOWN kernel subtracts from p on load
     double nb;                          // ||b||inf
     double tol;                         // stop tolerance of the running solve
     int cycle;                          // cycles completed in the running solve
