@@ -186,7 +186,7 @@ struct Impl {
 
 
     // ---- fused level halves (wl_fused3d.cuh) ---------------------------------------------------------------------
-    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = 16, FPF = 3;
+    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? 16 : 14, FPF = 3;   // 12 warps each
 
     // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
     // vectors; opt_fused == 1 keeps levels smaller than one tile on the generic kernels, 2 forces them (tests).
@@ -223,7 +223,19 @@ struct Impl {
             prm.N0 = f.g.N0; prm.N1 = f.g.N1; prm.N2 = f.g.N2;
             prm.tiles_x = (f.g.N0 + FTX - 1) / FTX;
             prm.tiles_y = (f.g.N1 + FTY - 1) / FTY;
-            prm.steps = (long long)prm.tiles_x * prm.tiles_y * f.g.N2;
+            // z-chunks: minimise waves * (planes per item + 6 run-in planes) over the chunk count (items dealt round-robin)
+            const long long ntiles = (long long)prm.tiles_x * prm.tiles_y;
+            const int half = f.g.N2 / 2;
+            long long best_cost = -1;
+            int best_nc = 1;
+            for (int nc = 1; nc <= half && nc <= 4096; ++nc) {
+                if (half / nc < 4 && nc > 1) break;                           // at least 8 planes per item
+                const long long items = ntiles * nc;
+                const long long waves = (items + c->num_sms - 1) / c->num_sms;
+                const long long cost = waves * (2LL * ((half + nc - 1) / nc) + 6);
+                if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_nc = nc; }
+            }
+            prm.nchunks = best_nc;
             prm.xout = P(x_out);
             prm.bc = P(bc);
             prm.scal = c->d_scal;
@@ -235,8 +247,7 @@ struct Impl {
                 CU(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                 attr_set = true;
             }
-            long long g = prm.steps / 8;
-            if (g < 1) g = 1;
+            long long g = ntiles * best_nc;
             if (g > c->num_sms) g = c->num_sms;
             if (NORMS && g > kMaxPartials) g = kMaxPartials;
             c->fused_grid = (int)g;
