@@ -243,18 +243,18 @@ def main():
                     e2e_ms.append(e0.elapsed_time(e1))
             e2e_total = float(np.sum(e2e_ms))
 
-        # V-cycle alone (graph launches back to back, no readback) and the dominant kernels alone
+        # V-cycles alone: wl_solve with tol = 0 runs exactly `reps` cycles (one graph launch + one 8-byte readback each,
+        # mean shift deferred into the next cycle); the dominant kernels alone follow
         bd = pr.empty_cells()
         wl.wl_divergence(pr.ctx, u0, bd)
-        p.zero_()
-        for _ in range(3):
-            wl.wl_vcycle(pr.ctx, p, bd, want_norm=False)
         reps = max(5, args.kernel_reps)
+        p.zero_()
+        wl.wl_solve(pr.ctx, p, bd, 0.0, 3)
+        p.zero_()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         e0.record(stream)
-        for _ in range(reps):
-            wl.wl_vcycle(pr.ctx, p, bd, want_norm=False)
+        wl.wl_solve(pr.ctx, p, bd, 0.0, reps)
         e1.record(stream)
         e1.synchronize()
         vcycle_ms = e0.elapsed_time(e1) / reps

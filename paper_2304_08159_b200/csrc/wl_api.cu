@@ -13,6 +13,7 @@
 #include "wl_common.cuh"
 #include "wl_generic.cuh"
 #include "wl_fused3d.cuh"
+#include "wl_tail.cuh"
 
 using namespace wl;
 
@@ -21,6 +22,7 @@ namespace {
 constexpr int kMaxLevels = 32;
 constexpr int kBlock = 256;
 constexpr int kMaxPartials = 148 * 16;
+constexpr int kTailSmemBudget = 200 * 1024;
 
 struct Level {
     Grid g;
@@ -52,6 +54,15 @@ struct wl_ctx {
     bool have_coeff = false;
     int opt_fused = 1, opt_graph = 1, opt_coarse_cta = 1;
     int num_sms = 148;
+    // cached CUDA graph of one V-cycle (H9), valid for one (p, b, variant, stream, options) combination
+    cudaStream_t own_stream = nullptr;   // the legacy default stream cannot be captured: graphs then run here, fenced by events
+    cudaEvent_t ev_in = nullptr, ev_out = nullptr;
+    cudaGraphExec_t cg_exec = nullptr;
+    void* cg_p = nullptr;
+    const void* cg_b = nullptr;
+    int cg_variant = -1;
+    int64_t cg_nodes = 0;
+    int tail_first = kMaxLevels; // first level of the single-CTA coarse tail (>= nlev: none fits shared memory)
     int fused_grid = 0;          // CTAs of the last fused launch (= number of sum partials it wrote)
     int64_t launches = 0;
     char err[256] = "";
@@ -195,7 +206,7 @@ struct Impl {
         const Grid& g = c->lev[l].g;
         constexpr int VEC = 16 / (int)sizeof(T);
         if (g.N0 % (2 * VEC)) return false;
-        if (c->opt_fused == 1 && (g.N0 < FTX || g.N1 < FTY || g.N2 < 8)) return false;
+        if (c->opt_fused == 1 && (g.N0 < FTX / 2 || g.N1 < 16 || g.N2 < 8)) return false;
         return get_encode_tiled() != nullptr;
     }
 
@@ -242,11 +253,6 @@ struct Impl {
             prm.partials = c->d_partials;
             auto kern = k_fused3d<T, FTX, FTY, FPF, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS>;
             constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF, PROLONG>();
-            static bool attr_set = false;
-            if (!attr_set) {
-                CU(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                attr_set = true;
-            }
             long long g = ntiles * best_nc;
             if (g > c->num_sms) g = c->num_sms;
             if (NORMS && g > kMaxPartials) g = kMaxPartials;
@@ -260,8 +266,9 @@ struct Impl {
     }
 
     // DOWN half of level l: x_out = J(J(x_in)) (x_in == nullptr: from zero), bc = R(b - A x_out).
-    static int down(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out, void* bc) {
-        if (!fused_ok(c, l)) return down_generic(c, l, x_in, b, x_out, bc);
+    static int down(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out, void* bc, bool shift = false) {
+        if (!fused_ok(c, l)) return shift ? fail(c, WL_EINVAL, "deferred mean shift needs the fused level-0 kernel") : down_generic(c, l, x_in, b, x_out, bc);
+        if (x_in && shift) return launch_fused<false, false, true, true, true, false>(c, l, x_in, nullptr, b, x_out, bc);
         if (x_in) return launch_fused<false, false, false, true, true, false>(c, l, x_in, nullptr, b, x_out, bc);
         return launch_fused<false, true, false, true, true, false>(c, l, nullptr, nullptr, b, x_out, bc);
     }
@@ -280,6 +287,30 @@ struct Impl {
         if (rc) return rc;
         k_finish_mean<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_partials, c->fused_grid, c->lev[0].g.M);
         KCHECK(c, "k_finish_mean");
+        return WL_OK;
+    }
+
+
+    // VCYCLE(l) for a level inside the coarse tail: one persistent CTA (wl_tail.cuh).  x_in == nullptr: zero guess.
+    static int tail(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out) {
+        TailParams<T> prm;
+        prm.nl = c->nlev - l;
+        prm.zero_in = x_in ? 0 : 1;
+        prm.coarsest_is_correction = (c->nlev > 1) ? 1 : 0;
+        unsigned off = 0;
+        for (int k = 0; k < prm.nl; ++k) {
+            const Level& v = c->lev[l + k];
+            prm.g[k] = v.g;
+            prm.L[k] = P(v.L);
+            prm.off[k] = off;
+            off += (unsigned)(((size_t)(3 + ND) * v.g.M * sizeof(T) + 15) / 16 * 16);
+        }
+        prm.x_in = P(x_in);
+        prm.b_in = P(b);
+        prm.x_out = P(x_out);
+        auto kern = k_coarse_tail<T, ND>;
+        kern<<<1, kTailThreads, off, c->stream>>>(prm);
+        KCHECK(c, "k_coarse_tail");
         return WL_OK;
     }
 
@@ -305,14 +336,19 @@ struct Impl {
 
     // VCYCLE(l): x_out = cycle(x_in) on level l; x_mid = level-sized scratch (may not alias x_in / x_out).
     // x_in == nullptr means a zero initial guess (every correction level).  norms: level-0 reductions after the UP half.
-    static int vcycle(wl_ctx* c, int l, const void* x_in, const void* b, void* x_mid, void* x_out, bool norms) {
+    static int vcycle(wl_ctx* c, int l, const void* x_in, const void* b, void* x_mid, void* x_out, bool norms, bool shift = false) {
         int rc;
+        if (c->opt_coarse_cta && l >= c->tail_first) {
+            const void* xi = (l == c->nlev - 1 && l > 0) ? nullptr : x_in;
+            if ((rc = tail(c, l, xi, b, x_out))) return rc;
+            return norms ? resnorm(c, x_out, b) : WL_OK;
+        }
         if (l == c->nlev - 1) {
             if ((rc = coarsest(c, l, (c->nlev > 1 && l > 0) ? nullptr : x_in, b, x_mid, x_out))) return rc;
             return norms ? resnorm(c, x_out, b) : WL_OK;
         }
         Level& k = c->lev[l + 1];
-        if ((rc = down(c, l, x_in, b, x_mid, k.b))) return rc;
+        if ((rc = down(c, l, x_in, b, x_mid, k.b, shift))) return rc;
         if ((rc = vcycle(c, l + 1, nullptr, k.b, k.x[0], k.x[1], false))) return rc;
         return up(c, l, x_mid, k.x[1], b, x_out, norms);
     }
@@ -352,14 +388,50 @@ struct Impl {
         return WL_OK;
     }
 
-    // One V-cycle; ||b - A p||inf (slot 1) and mean(p) come out of the level-0 UP half; then p -= mean.  The norm is
-    // taken before the shift: A·1 = 0, so it differs from the oracle's (after the shift) by rounding only.
-    static int cycle(wl_ctx* c, void* p, const void* b) {
+    // The mean removal of cycle k can ride on cycle k+1: its level-0 DOWN kernel subtracts (T)mean from p on load (exactly
+    // the value the oracle stores), the last cycle's shift is applied by one k_shift pass.  Needs the fused level 0.
+    static bool can_defer(const wl_ctx* c) { return c->nlev > 1 && c->tail_first > 0 && fused_ok(c, 0); }
+
+    // Generic-path scratch is allocated before a stream capture starts.
+    static int prepare(wl_ctx* c) {
+        for (int l = 0; l + 1 < c->nlev && l < (c->opt_coarse_cta ? c->tail_first : c->nlev); ++l)
+            if (!fused_ok(c, l)) { int rc = ensure_tmp(c, l); if (rc) return rc; }
+        if (!(c->opt_coarse_cta && c->tail_first < c->nlev)) { /* coarsest level runs on the generic kernels */ }
+        return WL_OK;
+    }
+
+    // One V-cycle; ||b - A p||inf (slot 1) and mean(p) come out of the level-0 UP half.  The norm is taken before the
+    // shift: A·1 = 0, so it differs from the oracle's (after the shift) by rounding only.
+    // deferred: p enters unshifted (scal->shift pending) and leaves unshifted; k_cycle_end moves mean -> shift.
+    static int cycle(wl_ctx* c, void* p, const void* b, bool deferred) {
         int rc;
-        if ((rc = vcycle(c, 0, p, b, c->lev[0].x[1], p, true))) return rc;
+        if ((rc = vcycle(c, 0, p, b, c->lev[0].x[1], p, true, deferred))) return rc;
+        if (!deferred) {
+            const long long M = c->lev[0].g.M;
+            k_shift<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, P(p), c->d_scal);
+            KCHECK(c, "k_shift");
+        }
+        return WL_OK;
+    }
+
+    static int apply_shift(wl_ctx* c, void* p) {
         const long long M = c->lev[0].g.M;
         k_shift<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, P(p), c->d_scal);
         KCHECK(c, "k_shift");
+        return WL_OK;
+    }
+
+    // Set every opt-in shared-memory size once, outside any stream capture.
+    static int init_kernels(wl_ctx* c) {
+        if constexpr (ND == 3) {
+            constexpr size_t s0 = fused3d_smem_bytes<T, FTX, FTY, FPF, false>(), s1 = fused3d_smem_bytes<T, FTX, FTY, FPF, true>();
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, false, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, false, true, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, true, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+        }
+        CU(c, cudaFuncSetAttribute(k_coarse_tail<T, ND>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTailSmemBudget));
         return WL_OK;
     }
 
@@ -406,6 +478,62 @@ int ensure_hist(wl_ctx* c, int maxcycles) {
     return WL_OK;
 }
 
+void drop_graph(wl_ctx* c) {
+    if (c->cg_exec) cudaGraphExecDestroy(c->cg_exec);
+    c->cg_exec = nullptr;
+    c->cg_variant = -1;
+}
+
+// One V-cycle (+ k_cycle_end bookkeeping when `in_solve`) on the ctx stream: a cached CUDA graph when WL_OPT_GRAPH is on.
+// variant: bit 0 = deferred mean shift, bit 1 = in_solve.
+int run_cycle(wl_ctx* c, void* p, const void* b, bool deferred, bool in_solve) {
+    int rc;
+    const int variant = (deferred ? 1 : 0) | (in_solve ? 2 : 0);
+    auto enqueue = [&]() -> int {
+        int r = DISPATCH(c, cycle)(c, p, b, deferred);
+        if (r) return r;
+        if (in_solve) {
+            k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, deferred ? 1 : 0);
+            KCHECK(c, "k_cycle_end");
+        }
+        return WL_OK;
+    };
+    if (!c->opt_graph) return enqueue();
+    cudaStream_t user = c->stream;
+    const bool proxy = (user == nullptr || user == cudaStreamLegacy || user == cudaStreamPerThread);
+    cudaStream_t gs = proxy ? c->own_stream : user;
+    if (!(c->cg_exec && c->cg_p == p && c->cg_b == b && c->cg_variant == variant)) {
+        drop_graph(c);
+        if ((rc = DISPATCH(c, prepare)(c))) return rc;
+        const int64_t before = c->launches;
+        CU(c, cudaStreamBeginCapture(gs, cudaStreamCaptureModeThreadLocal));
+        c->stream = gs;
+        rc = enqueue();
+        c->stream = user;
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamEndCapture(gs, &graph);
+        c->cg_nodes = c->launches - before;
+        c->launches = before;
+        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) return fail(c, WL_ECUDA, "cudaStreamEndCapture", e);
+        e = cudaGraphInstantiate(&c->cg_exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) { c->cg_exec = nullptr; return fail(c, WL_ECUDA, "cudaGraphInstantiate", e); }
+        c->cg_p = p; c->cg_b = b; c->cg_variant = variant;
+    }
+    if (proxy) {
+        CU(c, cudaEventRecord(c->ev_in, user));
+        CU(c, cudaStreamWaitEvent(gs, c->ev_in, 0));
+    }
+    CU(c, cudaGraphLaunch(c->cg_exec, gs));
+    if (proxy) {
+        CU(c, cudaEventRecord(c->ev_out, gs));
+        CU(c, cudaStreamWaitEvent(user, c->ev_out, 0));
+    }
+    c->launches += c->cg_nodes;
+    return WL_OK;
+}
+
 int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, double* hist, int* ncycles) {
     int rc;
     if ((rc = ensure_hist(c, maxcycles))) return rc;
@@ -416,19 +544,20 @@ int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, dou
     if ((rc = read_scalars(c))) return rc;
     const double nb = c->h_scal->nb;
     hist[0] = bits_to_double(c->h_scal->absmax_bits[1]);
+    const bool deferred = DISPATCH(c, can_defer)(c);
     int k = 0;
     while (k < maxcycles && hist[k] > tol * nb) {
-        if ((rc = DISPATCH(c, cycle)(c, p, b))) return rc;
-        k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist);
-        KCHECK(c, "k_cycle_end");
+        if ((rc = run_cycle(c, p, b, deferred, true))) return rc;
         if ((rc = read_scalars(c))) return rc;
         ++k;
         hist[k] = bits_to_double(c->h_scal->absmax_bits[1]);
     }
     if (k == 0) {
         if ((rc = DISPATCH(c, remove_mean)(c, p))) return rc;
-        CU(c, cudaStreamSynchronize(c->stream));
+    } else if (deferred) {
+        if ((rc = DISPATCH(c, apply_shift)(c, p))) return rc;
     }
+    CU(c, cudaStreamSynchronize(c->stream));
     *ncycles = k;
     return (hist[k] > tol * nb) ? WL_NOT_CONVERGED : WL_OK;
 }
@@ -482,6 +611,15 @@ int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
         for (int i = 0; i < ndim; ++i) N[i] /= 2;
     }
     c->nlev = nlev;
+    {   // coarse tail: the longest suffix of levels whose x ping-pong, b and L fit one CTA's shared memory
+        size_t need = 0;
+        c->tail_first = nlev;
+        for (int l = nlev - 1; l >= 0 && nlev - l <= kTailMaxLevels; --l) {
+            need += ((size_t)(3 + ndim) * c->lev[l].g.M * c->esz + 15) / 16 * 16;
+            if (need > (size_t)kTailSmemBudget) break;
+            c->tail_first = l;
+        }
+    }
 
     bool okm = true;
     auto dmalloc = [&](void** p, size_t bytes) {
@@ -505,10 +643,21 @@ int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
         snprintf(g_create_err, sizeof(g_create_err), "wl_create: cudaMallocHost failed");
     }
     if (okm && cudaMemset(c->d_scal, 0, sizeof(Scalars)) != cudaSuccess) okm = false;
+    if (okm && (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&c->ev_in, cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&c->ev_out, cudaEventDisableTiming) != cudaSuccess)) {
+        okm = false;
+        snprintf(g_create_err, sizeof(g_create_err), "wl_create: stream/event creation failed");
+    }
     if (!okm) {
         cudaGetLastError();
         wl_destroy(c);
         return WL_ENOMEM;
+    }
+    if (DISPATCH(c, init_kernels)(c) != WL_OK) {
+        snprintf(g_create_err, sizeof(g_create_err), "wl_create: %s", c->err);
+        wl_destroy(c);
+        return WL_ECUDA;
     }
     g_create_err[0] = 0;
     *out = c;
@@ -518,6 +667,10 @@ int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
 void wl_destroy(wl_ctx* c) {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
+    drop_graph(c);
+    if (c->own_stream) { cudaStreamSynchronize(c->own_stream); cudaStreamDestroy(c->own_stream); }
+    if (c->ev_in) cudaEventDestroy(c->ev_in);
+    if (c->ev_out) cudaEventDestroy(c->ev_out);
     for (int l = 0; l < kMaxLevels; ++l) {
         Level& v = c->lev[l];
         if (v.L) cudaFree(v.L);
@@ -541,12 +694,14 @@ void wl_destroy(wl_ctx* c) {
 
 int wl_set_stream(wl_ctx* c, void* s) {
     if (!c) return WL_EINVAL;
+    if (c->stream != (cudaStream_t)s) drop_graph(c);
     c->stream = (cudaStream_t)s;
     return WL_OK;
 }
 
 int wl_set_option(wl_ctx* c, int key, int value) {
     if (!c) return WL_EINVAL;
+    drop_graph(c);
     switch (key) {
         case WL_OPT_FUSED: c->opt_fused = (value < 0 || value > 2) ? 1 : value; return WL_OK;
         case WL_OPT_GRAPH: c->opt_graph = value ? 1 : 0; return WL_OK;
@@ -565,7 +720,7 @@ int wl_vcycle(wl_ctx* c, void* p, const void* b, double* rnorm_out) {
     if (!c) return WL_EINVAL;
     if (!p || !b) return fail(c, WL_EINVAL, "wl_vcycle: null pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle: coefficients not set");
-    int rc = DISPATCH(c, cycle)(c, p, b);
+    int rc = run_cycle(c, p, b, false, false);
     if (rc) return rc;
     if (rnorm_out) {
         if ((rc = read_scalars(c))) return rc;
@@ -655,7 +810,7 @@ int wl_down(wl_ctx* c, int level, const void* x_in, const void* b, void* x_out, 
     if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_down: bad level") : WL_EINVAL;
     if (!b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_down: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_down: coefficients not set");
-    return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
+    return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b, false);
 }
 
 int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b, void* x_out) {
@@ -669,7 +824,7 @@ int wl_vcycle_level(wl_ctx* c, int level, void* x, const void* b) {
     if (level_check(c, level, false)) return c ? fail(c, WL_EINVAL, "wl_vcycle_level: bad level") : WL_EINVAL;
     if (!x || !b) return fail(c, WL_EINVAL, "wl_vcycle_level: null pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle_level: coefficients not set");
-    return DISPATCH(c, vcycle)(c, level, x, b, level == 0 ? c->lev[0].x[1] : c->lev[level].x[0], x, false);
+    return DISPATCH(c, vcycle)(c, level, x, b, level == 0 ? c->lev[0].x[1] : c->lev[level].x[0], x, false, false);
 }
 
 int wl_residual_norm(wl_ctx* c, const void* p, const void* b, double* rnorm_out, double* mean_out) {

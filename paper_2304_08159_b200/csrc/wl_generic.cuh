@@ -307,12 +307,14 @@ __global__ void k_solve_begin(Scalars* scal, double* __restrict__ hist, double t
         scal->tol = tol;
         scal->maxcycles = maxcycles;
         scal->cycle = 0;
+        scal->shift = 0.0;
         scal->done = (r0 > tol * scal->nb && maxcycles > 0) ? 0 : 1;
     }
 }
-__global__ void k_cycle_end(Scalars* scal, double* __restrict__ hist) {
+__global__ void k_cycle_end(Scalars* scal, double* __restrict__ hist, int deferred) {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         if (scal->done) return;  // a speculative cycle after convergence changes nothing
+        scal->shift = deferred ? scal->mean_p : 0.0;  // what the next level-0 DOWN kernel subtracts on load
         const int k = scal->cycle + 1;
         const double r = __longlong_as_double((long long)scal->absmax_bits[1]);
         scal->cycle = k;
