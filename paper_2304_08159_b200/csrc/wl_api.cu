@@ -240,7 +240,7 @@ struct Impl {
             long long best_cost = -1;
             int best_nc = 1;
             for (int nc = 1; nc <= half && nc <= 4096; ++nc) {
-                if (half / nc < 4 && nc > 1) break;                           // at least 8 planes per item
+                if (half / nc < 1 && nc > 1) break;                           // at least 2 planes per item
                 const long long items = ntiles * nc;
                 const long long waves = (items + c->num_sms - 1) / c->num_sms;
                 const long long cost = waves * (2LL * ((half + nc - 1) / nc) + 6);
@@ -303,7 +303,7 @@ struct Impl {
             prm.g[k] = v.g;
             prm.L[k] = P(v.L);
             prm.off[k] = off;
-            off += (unsigned)(((size_t)(3 + ND) * v.g.M * sizeof(T) + 15) / 16 * 16);
+            off += (unsigned)(((size_t)(4 + ND) * v.g.M * sizeof(T) + 15) / 16 * 16);
         }
         prm.x_in = P(x_in);
         prm.b_in = P(b);
@@ -615,7 +615,7 @@ int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
         size_t need = 0;
         c->tail_first = nlev;
         for (int l = nlev - 1; l >= 0 && nlev - l <= kTailMaxLevels; --l) {
-            need += ((size_t)(3 + ndim) * c->lev[l].g.M * c->esz + 15) / 16 * 16;
+            need += ((size_t)(4 + ndim) * c->lev[l].g.M * c->esz + 15) / 16 * 16;
             if (need > (size_t)kTailSmemBudget) break;
             c->tail_first = l;
         }
