@@ -51,6 +51,27 @@ def _peaks():
         return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
+def max_over_ranks(values, device=None):
+    """Element-wise MAX of a list of floats over all ranks of the default process group (identity at world size 1).
+    The only collective of the N > 1 ("replicas only") path; works on NCCL (device tensor) and on gloo (CPU)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def whole_job_value(world: int, cells: int, cycles: int, seconds_per_step: float) -> float:
+    """Fine cells per second per V-cycle, summed over the `world` replicas (each rank projects its own grid)."""
+    return world * cells * cycles / seconds_per_step if (cycles > 0 and seconds_per_step > 0) else 0.0
+
+
+# DRAM traffic of one level-0 DOWN launch at 512^3 fp32 from the last `ncu --set full` capture (profiles/): bytes.
+NCU_TRAFFIC_DOWN_512 = None
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -278,21 +299,21 @@ def main():
 
     # max over ranks
     if world > 1:
-        t = torch.tensor([total_ms, 0.0 if args.no_e2e else e2e_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t[0].item())
+        red = max_over_ranks([total_ms, 0.0 if args.no_e2e else e2e_total], dev)
+        total_ms = red[0]
         if not args.no_e2e:
-            e2e_total = float(t[1].item())
+            e2e_total = red[1]
 
     sec_per_step = total_ms / 1e3 / args.steps
-    value = world * M * nc / sec_per_step if nc > 0 else 0.0
+    value = whole_job_value(world, M, int(nc), sec_per_step)
     peak, peak_src = _peaks()
     roof = None
     if kern:
         bytes_down = _algorithmic_bytes_down(n, esz) * M
         ach = bytes_down / (kern["down"]["ms"] * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": "level-0 DOWN (2 pre-sweeps + residual + restriction), via wl_down",
-                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": NCU_TRAFFIC_DOWN_512 if (args.config == 4 and args.scale == 1 and dt == np.float32) else None,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_down,
                 "launches_per_call": kern["down"]["launches_per_call"], "ms": kern["down"]["ms"],
                 "up_kernel": {"ms": kern["up"]["ms"], "achieved": bytes_down / (kern["up"]["ms"] * 1e-3) / 1e9,
@@ -316,7 +337,7 @@ def main():
         e2e_sec = e2e_total / 1e3 / args.steps
         h2d = u_host.numel() * esz + L_host.numel() * esz + M * esz
         d2h = u_host.numel() * esz + M * esz
-        line["e2e"] = {"value": world * M * nc2 / e2e_sec, "unit": UNIT, "ms_per_step": e2e_sec * 1e3,
+        line["e2e"] = {"value": whole_job_value(world, M, int(nc2), e2e_sec), "unit": UNIT, "ms_per_step": e2e_sec * 1e3,
                        "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -14,6 +14,7 @@
 #include "wl_generic.cuh"
 #include "wl_fused3d.cuh"
 #include "wl_tail.cuh"
+#include "wl_rows.cuh"
 
 using namespace wl;
 
@@ -63,6 +64,7 @@ struct wl_ctx {
     int cg_variant = -1;
     int64_t cg_nodes = 0;
     int tail_first = kMaxLevels; // first level of the single-CTA coarse tail (>= nlev: none fits shared memory)
+    int check_done = 0;          // set while enqueuing a solve cycle: kernels that can, return at once when scal->done
     int fused_grid = 0;          // CTAs of the last fused launch (= number of sum partials it wrote)
     int64_t launches = 0;
     char err[256] = "";
@@ -109,10 +111,26 @@ struct Impl {
     static T* P(void* p) { return (T*)p; }
     static const T* P(const void* p) { return (const T*)p; }
 
+    // Row-wise 16-byte kernels need whole vectors per row and aligned arrays.
+    static bool rows_ok(const Grid& g, const void* a, const void* b2 = nullptr, const void* c2 = nullptr) {
+        constexpr int VEC = 16 / (int)sizeof(T);
+        return g.N0 % VEC == 0 && (((uintptr_t)a | (uintptr_t)b2 | (uintptr_t)c2) & 15) == 0;
+    }
+    static int rows_grid(const wl_ctx* c, long long nrows) {
+        long long blocks = (nrows + kRowsY - 1) / kRowsY;
+        const long long cap = (long long)c->num_sms * 8;
+        return (int)(blocks < 1 ? 1 : (blocks < cap ? blocks : cap));
+    }
+
     static int set_coeff(wl_ctx* c, const void* Ldev) {
         Level& f = c->lev[0];
-        k_copy_coeff<T, ND><<<grid_for(c, f.g.M * ND), kBlock, 0, c->stream>>>(f.g, P(Ldev), P(f.L));
-        KCHECK(c, "k_copy_coeff");
+        if (rows_ok(f.g, Ldev, f.L)) {
+            k_copy_coeff_rows<T, ND><<<rows_grid(c, (long long)f.g.N1 * f.g.N2 * ND), dim3(kRowsX, kRowsY), 0, c->stream>>>(f.g, P(Ldev), P(f.L));
+            KCHECK(c, "k_copy_coeff_rows");
+        } else {
+            k_copy_coeff<T, ND><<<grid_for(c, f.g.M * ND), kBlock, 0, c->stream>>>(f.g, P(Ldev), P(f.L));
+            KCHECK(c, "k_copy_coeff");
+        }
         for (int l = 0; l + 1 < c->nlev; ++l) {
             Level& a = c->lev[l];
             Level& b = c->lev[l + 1];
@@ -251,6 +269,7 @@ struct Impl {
             prm.bc = P(bc);
             prm.scal = c->d_scal;
             prm.partials = c->d_partials;
+            prm.check_done = c->check_done;
             auto kern = k_fused3d<T, FTX, FTY, FPF, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS>;
             constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF, PROLONG>();
             long long g = ntiles * best_nc;
@@ -308,6 +327,8 @@ struct Impl {
         prm.x_in = P(x_in);
         prm.b_in = P(b);
         prm.x_out = P(x_out);
+        prm.scal = c->d_scal;
+        prm.check_done = c->check_done;
         auto kern = k_coarse_tail<T, ND>;
         kern<<<1, kTailThreads, off, c->stream>>>(prm);
         KCHECK(c, "k_coarse_tail");
@@ -392,6 +413,15 @@ struct Impl {
     // the value the oracle stores), the last cycle's shift is applied by one k_shift pass.  Needs the fused level 0.
     static bool can_defer(const wl_ctx* c) { return c->nlev > 1 && c->tail_first > 0 && fused_ok(c, 0); }
 
+    // A cycle may be enqueued before the previous one's stop test is known only if every kernel of it that writes
+    // the iterate checks scal->done: all levels above the tail fused, the rest in the tail CTA.
+    static bool can_speculate(const wl_ctx* c) {
+        if (!c->opt_coarse_cta || c->tail_first >= c->nlev || c->tail_first == 0) return false;
+        for (int l = 0; l < c->tail_first; ++l)
+            if (!fused_ok(c, l)) return false;
+        return true;
+    }
+
     // Generic-path scratch is allocated before a stream capture starts.
     static int prepare(wl_ctx* c) {
         for (int l = 0; l + 1 < c->nlev && l < (c->opt_coarse_cta ? c->tail_first : c->nlev); ++l)
@@ -437,6 +467,11 @@ struct Impl {
 
     static int divergence(wl_ctx* c, const void* u, void* b) {
         Level& f = c->lev[0];
+        if (rows_ok(f.g, u, b)) {
+            k_divergence_rows<T, ND><<<rows_grid(c, (long long)f.g.N1 * f.g.N2), dim3(kRowsX, kRowsY), 0, c->stream>>>(f.g, P(u), P(b));
+            KCHECK(c, "k_divergence_rows");
+            return WL_OK;
+        }
         k_divergence<T, ND><<<grid_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, P(u), P(b));
         KCHECK(c, "k_divergence");
         return WL_OK;
@@ -444,6 +479,11 @@ struct Impl {
 
     static int gradient(wl_ctx* c, void* u, const void* p) {
         Level& f = c->lev[0];
+        if (rows_ok(f.g, u, p, f.L)) {
+            k_gradient_rows<T, ND><<<rows_grid(c, (long long)f.g.N1 * f.g.N2), dim3(kRowsX, kRowsY), 0, c->stream>>>(f.g, P(f.L), P(u), P(p));
+            KCHECK(c, "k_gradient_rows");
+            return WL_OK;
+        }
         k_gradient<T, ND><<<grid_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, P(f.L), P(u), P(p));
         KCHECK(c, "k_gradient");
         return WL_OK;
@@ -466,8 +506,11 @@ inline double bits_to_double(unsigned long long b) {
     return d;
 }
 
+void drop_graph(wl_ctx* c);
+
 int ensure_hist(wl_ctx* c, int maxcycles) {
     if (maxcycles + 1 <= c->hist_cap) return WL_OK;
+    drop_graph(c);   // the cached graph holds the old history pointers
     if (c->d_hist) cudaFree(c->d_hist);
     if (c->h_hist) cudaFreeHost(c->h_hist);
     c->d_hist = nullptr; c->h_hist = nullptr; c->hist_cap = 0;
@@ -490,10 +533,12 @@ int run_cycle(wl_ctx* c, void* p, const void* b, bool deferred, bool in_solve) {
     int rc;
     const int variant = (deferred ? 1 : 0) | (in_solve ? 2 : 0);
     auto enqueue = [&]() -> int {
+        c->check_done = in_solve ? 1 : 0;
         int r = DISPATCH(c, cycle)(c, p, b, deferred);
+        c->check_done = 0;
         if (r) return r;
         if (in_solve) {
-            k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, deferred ? 1 : 0);
+            k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, deferred ? 1 : 0, c->h_scal, c->h_hist);
             KCHECK(c, "k_cycle_end");
         }
         return WL_OK;
@@ -534,6 +579,26 @@ int run_cycle(wl_ctx* c, void* p, const void* b, bool deferred, bool in_solve) {
     return WL_OK;
 }
 
+// Spin on the pinned mirror until cycle `target` has been recorded by k_cycle_end; checks the stream now and then so a
+// faulted or drained stream cannot hang the host.
+int wait_cycle(wl_ctx* c, int target) {
+    volatile Scalars* hm = c->h_scal;
+    cudaStream_t user = c->stream;
+    const bool proxy = c->opt_graph && (user == nullptr || user == cudaStreamLegacy || user == cudaStreamPerThread);
+    cudaStream_t gs = proxy ? c->own_stream : user;
+    for (unsigned spins = 0;; ++spins) {
+        if (hm->cycle >= target) return WL_OK;
+        if ((spins & 0xfff) == 0xfff) {
+            cudaError_t e = cudaStreamQuery(gs);
+            if (e == cudaSuccess) {
+                if (hm->cycle >= target) return WL_OK;
+                return fail(c, WL_ECUDA, "wl_solve: the stream drained without recording the cycle");
+            }
+            if (e != cudaErrorNotReady) return fail(c, WL_ECUDA, "wl_solve: cudaStreamQuery", e);
+        }
+    }
+}
+
 int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, double* hist, int* ncycles) {
     int rc;
     if ((rc = ensure_hist(c, maxcycles))) return rc;
@@ -545,12 +610,22 @@ int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, dou
     const double nb = c->h_scal->nb;
     hist[0] = bits_to_double(c->h_scal->absmax_bits[1]);
     const bool deferred = DISPATCH(c, can_defer)(c);
-    int k = 0;
-    while (k < maxcycles && hist[k] > tol * nb) {
-        if ((rc = run_cycle(c, p, b, deferred, true))) return rc;
-        if ((rc = read_scalars(c))) return rc;
+    // Cycles are enqueued up to `depth` ahead of the stop test; the host polls the pinned mirror k_cycle_end writes
+    // instead of synchronising the stream, so the GPU does not idle for a host round trip per cycle.
+    const int depth = DISPATCH(c, can_speculate)(c) ? 2 : 1;
+    volatile Scalars* hm = c->h_scal;
+    hm->cycle = 0;
+    int launched = 0, k = 0;
+    bool stop = !(maxcycles > 0 && hist[0] > tol * nb);
+    while (!stop) {
+        while (launched < maxcycles && launched - k < depth) {
+            if ((rc = run_cycle(c, p, b, deferred, true))) return rc;
+            ++launched;
+        }
+        if ((rc = wait_cycle(c, k + 1))) return rc;
         ++k;
-        hist[k] = bits_to_double(c->h_scal->absmax_bits[1]);
+        hist[k] = c->h_hist[k];
+        if (!(hist[k] > tol * nb) || k >= maxcycles) stop = true;
     }
     if (k == 0) {
         if ((rc = DISPATCH(c, remove_mean)(c, p))) return rc;

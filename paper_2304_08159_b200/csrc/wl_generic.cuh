@@ -311,7 +311,8 @@ __global__ void k_solve_begin(Scalars* scal, double* __restrict__ hist, double t
         scal->done = (r0 > tol * scal->nb && maxcycles > 0) ? 0 : 1;
     }
 }
-__global__ void k_cycle_end(Scalars* scal, double* __restrict__ hist, int deferred) {
+__global__ void k_cycle_end(Scalars* scal, double* __restrict__ hist, int deferred, Scalars* host_mirror,
+                            double* host_hist) {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         if (scal->done) return;  // a speculative cycle after convergence changes nothing
         scal->shift = deferred ? scal->mean_p : 0.0;  // what the next level-0 DOWN kernel subtracts on load
@@ -319,7 +320,12 @@ __global__ void k_cycle_end(Scalars* scal, double* __restrict__ hist, int deferr
         const double r = __longlong_as_double((long long)scal->absmax_bits[1]);
         scal->cycle = k;
         hist[k] = r;
-        if (!(r > scal->tol * scal->nb) || k >= scal->maxcycles) scal->done = 1;
+        const int done = (!(r > scal->tol * scal->nb) || k >= scal->maxcycles) ? 1 : 0;
+        if (done) scal->done = 1;
+        // pinned host mirror (device-mapped): the host polls `cycle` instead of synchronising the stream
+        host_hist[k] = r;
+        __threadfence_system();
+        *((volatile int*)&host_mirror->cycle) = k;
     }
 }
 

@@ -23,6 +23,8 @@ struct TailParams {
     const T* b_in;                   // tail level 0 right-hand side (global)
     T* x_out;                        // tail level 0 result (global)
     int coarsest_is_correction;      // 1: the coarsest level starts from 0 (it is a correction level of the hierarchy)
+    const Scalars* scal;             // with check_done: return at once if scal->done (speculative cycle past convergence)
+    int check_done;
 };
 
 // Named barrier over the first `nthreads` threads of the CTA (a multiple of 32): small levels do not make the whole
@@ -52,6 +54,7 @@ __device__ __forceinline__ void tail_sweep(const Grid& g, const T* L, const T* C
 
 template <typename T, int ND>
 __global__ void __launch_bounds__(kTailThreads, 1) k_coarse_tail(TailParams<T> P) {
+    if (P.check_done && P.scal->done) return;
     extern __shared__ __align__(16) unsigned char tail_smem[];
     auto XA = [&](int l) -> T* { return (T*)(tail_smem + P.off[l]); };
     auto XB = [&](int l) -> T* { return XA(l) + P.g[l].M; };
