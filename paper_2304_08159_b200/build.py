@@ -19,6 +19,10 @@ NVCC_FLAGS = [
     "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared",
     "-cudart", "static",
+    # No FMA contraction: every multiply and add rounds separately, exactly as the oracle's (-ffp-contract=off), which
+    # makes the fp32 and fp64 iterates and residual histories bit-identical to it (DESIGN.md §3 reading 12; measured
+    # cost: 5 % of the 512^3 V-cycle).  Explicit fmaf() calls (the reciprocal's Newton steps) stay fused.
+    "-fmad=false",
 ]
 
 

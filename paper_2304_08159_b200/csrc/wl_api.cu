@@ -13,6 +13,7 @@
 #include "wl_common.cuh"
 #include "wl_generic.cuh"
 #include "wl_fused3d.cuh"
+#include "wl_fused2d.cuh"
 #include "wl_tail.cuh"
 #include "wl_rows.cuh"
 
@@ -22,7 +23,7 @@ namespace {
 
 constexpr int kMaxLevels = 32;
 constexpr int kBlock = 256;
-constexpr int kMaxPartials = 148 * 16;
+constexpr int kMaxPartials = 1 << 15;   // per-CTA sum partials (fused 2-D kernels: one per tile)
 constexpr int kTailSmemBudget = 200 * 1024;
 
 struct Level {
@@ -219,13 +220,55 @@ struct Impl {
 
     // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
     // vectors; opt_fused == 1 keeps levels smaller than one tile on the generic kernels, 2 forces them (tests).
+    static constexpr int F2TX = sizeof(T) == 4 ? 64 : 32, F2TY = 32;   // 2-D tile
+
     static bool fused_ok(const wl_ctx* c, int l) {
-        if (ND != 3 || !c->opt_fused || l + 1 >= c->nlev) return false;
+        if (!c->opt_fused || l + 1 >= c->nlev) return false;
         const Grid& g = c->lev[l].g;
         constexpr int VEC = 16 / (int)sizeof(T);
         if (g.N0 % (2 * VEC)) return false;
-        if (c->opt_fused == 1 && (g.N0 < FTX / 2 || g.N1 < 16 || g.N2 < 8)) return false;
+        if (ND == 3) {
+            if (c->opt_fused == 1 && (g.N0 < FTX / 2 || g.N1 < 16 || g.N2 < 8)) return false;
+        } else {
+            if (c->opt_fused == 1 && (g.N0 < F2TX / 2 || g.N1 < F2TY / 2)) return false;
+            const long long tiles = (long long)((g.N0 + F2TX - 1) / F2TX) * ((g.N1 + F2TY - 1) / F2TY);
+            if (tiles > kMaxPartials) return false;
+        }
         return get_encode_tiled() != nullptr;
+    }
+
+    static bool map_cells2(CUtensorMap* m, const void* base, const Grid& g, bool coarse_box) {
+        using G = F2<T, F2TX, F2TY>;
+        if (((uintptr_t)base & 15) != 0) return false;
+        const uint64_t d[3] = {(uint64_t)g.N0, (uint64_t)g.N1, 1};
+        const uint32_t b[3] = {(uint32_t)(coarse_box ? G::CWX : G::WX), (uint32_t)(coarse_box ? G::CWY : G::WY), 1u};
+        return encode_map(m, base, (int)sizeof(T), 2, d, b);
+    }
+
+    template <bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS, bool RIN = false>
+    static int launch_fused2(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out, void* bc) {
+        using G = F2<T, F2TX, F2TY>;
+        Level& f = c->lev[l];
+        CUtensorMap mx, mb, mL0, mL1, mxc;
+        bool ok = map_cells2(&mb, b, f.g, false) && map_cells2(&mL0, P(f.L), f.g, false) && map_cells2(&mL1, P(f.L) + f.g.M, f.g, false);
+        if (ZERO_IN) mx = mb; else ok = ok && map_cells2(&mx, x_in, f.g, false);
+        if (PROLONG) ok = ok && map_cells2(&mxc, xc, c->lev[l + 1].g, true); else mxc = mb;
+        if (!ok) return fail(c, WL_ECUDA, "cuTensorMapEncodeTiled refused a level array (alignment?)");
+        Fused2Params<T> prm;
+        prm.N0 = f.g.N0; prm.N1 = f.g.N1;
+        prm.tiles_x = (f.g.N0 + F2TX - 1) / F2TX;
+        prm.tiles_y = (f.g.N1 + F2TY - 1) / F2TY;
+        prm.xout = P(x_out);
+        prm.bc = P(bc);
+        prm.scal = c->d_scal;
+        prm.partials = c->d_partials;
+        prm.check_done = c->check_done;
+        const int grid = prm.tiles_x * prm.tiles_y;
+        c->fused_grid = grid;
+        k_fused2d<T, F2TX, F2TY, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN>
+            <<<grid, G::NT, fused2d_smem_bytes<T, F2TX, F2TY>(), c->stream>>>(mx, mb, mL0, mL1, mxc, prm);
+        KCHECK(c, "k_fused2d");
+        return WL_OK;
     }
 
     static bool map_cells(CUtensorMap* m, const void* base, const Grid& g, bool coarse_box) {
@@ -236,7 +279,7 @@ struct Impl {
         return encode_map(m, base, (int)sizeof(T), 3, d, b);
     }
 
-    template <bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS>
+    template <bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS, bool RIN = false>
     static int launch_fused(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out, void* bc) {
         if constexpr (ND == 3) {
             using G = F3<T, FTX, FTY>;
@@ -270,7 +313,7 @@ struct Impl {
             prm.scal = c->d_scal;
             prm.partials = c->d_partials;
             prm.check_done = c->check_done;
-            auto kern = k_fused3d<T, FTX, FTY, FPF, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS>;
+            auto kern = k_fused3d<T, FTX, FTY, FPF, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN>;
             constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF, PROLONG>();
             long long g = ntiles * best_nc;
             if (g > c->num_sms) g = c->num_sms;
@@ -280,7 +323,7 @@ struct Impl {
             KCHECK(c, "k_fused3d");
             return WL_OK;
         } else {
-            return fail(c, WL_EINVAL, "fused kernels are 3-D only");
+            return launch_fused2<PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN>(c, l, x_in, xc, b, x_out, bc);
         }
     }
 
@@ -435,19 +478,36 @@ struct Impl {
     // deferred: p enters unshifted (scal->shift pending) and leaves unshifted; k_cycle_end moves mean -> shift.
     static int cycle(wl_ctx* c, void* p, const void* b, bool deferred) {
         int rc;
-        if ((rc = vcycle(c, 0, p, b, c->lev[0].x[1], p, true, deferred))) return rc;
-        if (!deferred) {
-            const long long M = c->lev[0].g.M;
-            k_shift<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, P(p), c->d_scal);
-            KCHECK(c, "k_shift");
-        }
-        return WL_OK;
+        if (deferred) return vcycle(c, 0, p, b, c->lev[0].x[1], p, true, true);
+        // classic order, exactly the oracle's: V-cycle, p -= mean(p), then ||b - A p||inf of the shifted p
+        if ((rc = vcycle(c, 0, p, b, c->lev[0].x[1], p, false, false))) return rc;
+        if ((rc = remove_mean(c, p))) return rc;
+        return resnorm(c, p, b);
     }
 
     static int apply_shift(wl_ctx* c, void* p) {
         const long long M = c->lev[0].g.M;
         k_shift<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, P(p), c->d_scal);
         KCHECK(c, "k_shift");
+        return WL_OK;
+    }
+
+    // The solve cycle with the lagged stop test (k_cycle_check): DOWN0 measures the residual of its input for free, UP0
+    // needs no residual stage (2 stencil stages instead of 3) and only sums p.
+    static int cycle_lagged(wl_ctx* c, void* p, const void* b) {
+        int rc;
+        Level& k1 = c->lev[1];
+        k_zero_slot<<<1, 32, 0, c->stream>>>(c->d_scal, 1);
+        KCHECK(c, "k_zero_slot");
+        if ((rc = launch_fused<false, false, true, true, true, false, true>(c, 0, p, nullptr, b, c->lev[0].x[1], k1.b))) return rc;
+        k_cycle_check<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, c->h_scal, c->h_hist);
+        KCHECK(c, "k_cycle_check");
+        if ((rc = vcycle(c, 1, nullptr, k1.b, k1.x[0], k1.x[1], false, false))) return rc;
+        if ((rc = launch_fused<true, false, false, false, false, true, false>(c, 0, c->lev[0].x[1], k1.x[1], b, p, nullptr))) return rc;
+        k_finish_mean<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_partials, c->fused_grid, c->lev[0].g.M);
+        KCHECK(c, "k_finish_mean");
+        k_cycle_end_lagged<<<1, 32, 0, c->stream>>>(c->d_scal);
+        KCHECK(c, "k_cycle_end_lagged");
         return WL_OK;
     }
 
@@ -460,6 +520,18 @@ struct Impl {
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, true, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, false, true, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, true, false, false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+        }
+        if constexpr (ND == 2) {
+            constexpr int s2 = (int)fused2d_smem_bytes<T, F2TX, F2TY>();
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, true, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, true, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
         }
         CU(c, cudaFuncSetAttribute(k_coarse_tail<T, ND>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTailSmemBudget));
         return WL_OK;
@@ -529,15 +601,15 @@ void drop_graph(wl_ctx* c) {
 
 // One V-cycle (+ k_cycle_end bookkeeping when `in_solve`) on the ctx stream: a cached CUDA graph when WL_OPT_GRAPH is on.
 // variant: bit 0 = deferred mean shift, bit 1 = in_solve.
-int run_cycle(wl_ctx* c, void* p, const void* b, bool deferred, bool in_solve) {
+int run_cycle(wl_ctx* c, void* p, const void* b, bool deferred, bool in_solve, bool lagged = false) {
     int rc;
-    const int variant = (deferred ? 1 : 0) | (in_solve ? 2 : 0);
+    const int variant = (deferred ? 1 : 0) | (in_solve ? 2 : 0) | (lagged ? 4 : 0);
     auto enqueue = [&]() -> int {
         c->check_done = in_solve ? 1 : 0;
-        int r = DISPATCH(c, cycle)(c, p, b, deferred);
+        int r = lagged ? DISPATCH(c, cycle_lagged)(c, p, b) : DISPATCH(c, cycle)(c, p, b, deferred);
         c->check_done = 0;
         if (r) return r;
-        if (in_solve) {
+        if (in_solve && !lagged) {
             k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, deferred ? 1 : 0, c->h_scal, c->h_hist);
             KCHECK(c, "k_cycle_end");
         }
@@ -609,18 +681,27 @@ int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, dou
     if ((rc = read_scalars(c))) return rc;
     const double nb = c->h_scal->nb;
     hist[0] = bits_to_double(c->h_scal->absmax_bits[1]);
-    const bool deferred = DISPATCH(c, can_defer)(c);
+    const bool deferred = DISPATCH(c, can_defer)(c) && DISPATCH(c, can_speculate)(c);
     // Cycles are enqueued up to `depth` ahead of the stop test; the host polls the pinned mirror k_cycle_end writes
     // instead of synchronising the stream, so the GPU does not idle for a host round trip per cycle.
-    const int depth = DISPATCH(c, can_speculate)(c) ? 2 : 1;
+    const bool spec = DISPATCH(c, can_speculate)(c);
+    const bool lagged = deferred && spec;   // hist[k] is read off the DOWN kernel of launch k+1 (k_cycle_check)
+    const int depth = spec ? 2 : 1;
     volatile Scalars* hm = c->h_scal;
     hm->cycle = 0;
     int launched = 0, k = 0;
     bool stop = !(maxcycles > 0 && hist[0] > tol * nb);
     while (!stop) {
-        while (launched < maxcycles && launched - k < depth) {
-            if ((rc = run_cycle(c, p, b, deferred, true))) return rc;
-            ++launched;
+        if (lagged) {
+            while (launched < k + 2 && launched < maxcycles + 1) {
+                if ((rc = run_cycle(c, p, b, true, true, true))) return rc;
+                ++launched;
+            }
+        } else {
+            while (launched < maxcycles && launched - k < depth) {
+                if ((rc = run_cycle(c, p, b, deferred, true))) return rc;
+                ++launched;
+            }
         }
         if ((rc = wait_cycle(c, k + 1))) return rc;
         ++k;

@@ -234,3 +234,30 @@ def test_project_host_matches_device_call(env):
     assert nc_h == nc and rc_h == rc and np.array_equal(hist_h, hist)
     assert torch.equal(uh, ud.cpu()) and torch.equal(ph, p.cpu())
     pr.close()
+
+
+@pytest.mark.parametrize("config,scale,dt,K", [(0, 1, np.float32, 10), (1, 4, np.float32, 12), (2, 2, np.float32, 8),
+                                                (3, 4, np.float32, 6), (4, 8, np.float32, 8)])
+def test_bit_identical_iterates_and_history(env, config, scale, dt, K):
+    """Drift alarm, beyond BASELINE's tolerances: the library is compiled without FMA contraction and keeps the oracle's
+    expression order, so after K cycles p and every hist[k] equal the oracle's bit for bit (DESIGN.md §3 reading 12).
+    The mean is summed in fp64 in a different order on the GPU; its fp32 rounding can differ only with probability ~1e-9
+    (in fp64 the differently ordered sum itself shows in the last bits of p, so fp64 is held to 1e-10 only)."""
+    torch, wl = env["torch"], env["wl"]
+    cfg = env["synth"].make_config(config, dtype=dt, scale=scale)
+    L, u = cfg["L"].astype(dt), cfg["u"].astype(dt)
+    o = env["oracle"].Oracle(cfg["dims"], dt)
+    o.set_coeff(L)
+    b = o.divergence(u)
+    p_ref, hist_ref, _, _ = o.solve(np.zeros_like(b), b, 0.0, K)
+    pr = _projector(env, cfg, dt)
+    wl.wl_set_coeff(pr.ctx, torch.from_numpy(L).cuda())
+    bd = pr.empty_cells()
+    wl.wl_divergence(pr.ctx, torch.from_numpy(u).cuda(), bd)
+    assert bd.cpu().numpy().tobytes() == b.tobytes()
+    p = pr.zeros_cells()
+    hist, nc, rc = wl.wl_solve(pr.ctx, p, bd, 0.0, K)
+    assert nc == K
+    assert np.array_equal(hist, hist_ref), np.abs(hist / hist_ref - 1).max()
+    assert p.cpu().numpy().tobytes() == p_ref.tobytes()
+    pr.close()
