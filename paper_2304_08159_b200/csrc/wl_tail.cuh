@@ -33,6 +33,38 @@ __device__ __forceinline__ void bar_sync_n(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
+// 32-bit index helpers (tail levels have at most a few thousand cells): no 64-bit divisions in the sweeps.
+template <int ND>
+__device__ __forceinline__ void decompose_i(const Grid& g, int I, int& i0, int& i1, int& i2) {
+    const int q = I / g.N0;
+    i0 = I - q * g.N0;
+    if (ND == 3) {
+        const int q2 = q / g.N1;
+        i1 = q - q2 * g.N1;
+        i2 = q2;
+    } else {
+        i1 = q;
+        i2 = 0;
+    }
+}
+// A x at one cell, the oracle's term order (upper face, lower face; axis 0, 1, 2); absent neighbours are skipped.
+template <typename T, int ND>
+__device__ __forceinline__ T stencil_i(const Grid& g, const T* L, const T* x, int I, int i0, int i1, int i2) {
+    const int Ii[3] = {i0, i1, i2};
+    const int Ni[3] = {g.N0, g.N1, g.N2};
+    const int st[3] = {1, g.N0, g.N0 * g.N1};
+    const int M = (int)g.M;
+    const T xc = x[I];
+    T s = 0;
+#pragma unroll
+    for (int i = 0; i < ND; ++i) {
+        const T* Li = L + i * M;
+        if (Ii[i] + 1 < Ni[i]) s += Li[I + st[i]] * (x[I + st[i]] - xc);
+        if (Ii[i] > 0) s += Li[I] * (x[I - st[i]] - xc);
+    }
+    return s;
+}
+
 // One damped-Jacobi sweep over a level held in shared memory; C = omega * invD per cell (precomputed, same rounding as
 // the oracle's omega*invD).  Only threads < nthr take part (and synchronise).
 template <typename T, int ND>
@@ -43,13 +75,66 @@ __device__ __forceinline__ void tail_sweep(const Grid& g, const T* L, const T* C
             xout[I] = C[I] * ((T)0 - b[I]);
         } else {
             int i0, i1, i2;
-            decompose<T, ND>(g, I, i0, i1, i2);
-            T Ax, D;
-            stencil_cell<T, ND>(g, L, xin, I, i0, i1, i2, Ax, D);
+            decompose_i<ND>(g, I, i0, i1, i2);
+            const T Ax = stencil_i<T, ND>(g, L, xin, I, i0, i1, i2);
             xout[I] = xin[I] + C[I] * (Ax - b[I]);
         }
     }
     bar_sync_n(1, nthr);
+}
+
+// `sweeps` sweeps on a level with at most one cell per thread (the coarsest level): the cell's coefficients, neighbour
+// indices, omega/D and b stay in registers; a sweep is 2*ND shared loads, the stencil, one store and one barrier.
+// Starts from XA (or from zero), ping-pongs XA/XB, leaves the result in XA.  sweeps must be even.
+template <typename T, int ND>
+__device__ __forceinline__ void tail_sweeps_cached(const Grid& g, const T* L, const T* C, T* XA, T* XB, const T* b,
+                                                   bool from_zero, int sweeps, int nthr) {
+    const int I = threadIdx.x;
+    const bool has = I < (int)g.M;
+    const int M = (int)g.M;
+    T Lf[2 * ND];
+    int nb[2 * ND];
+    T cI = 0, bI = 0, xv = 0;
+    if (has) {
+        int i0, i1, i2;
+        decompose_i<ND>(g, I, i0, i1, i2);
+        const int Ii[3] = {i0, i1, i2};
+        const int Ni[3] = {g.N0, g.N1, g.N2};
+        const int st[3] = {1, g.N0, g.N0 * g.N1};
+#pragma unroll
+        for (int i = 0; i < ND; ++i) {
+            const bool up = Ii[i] + 1 < Ni[i], lo = Ii[i] > 0;
+            nb[2 * i] = up ? I + st[i] : -1;
+            nb[2 * i + 1] = lo ? I - st[i] : -1;
+            Lf[2 * i] = up ? L[i * M + I + st[i]] : (T)0;
+            Lf[2 * i + 1] = lo ? L[i * M + I] : (T)0;
+        }
+        cI = C[I];
+        bI = b[I];
+        xv = from_zero ? (T)0 : XA[I];
+    } else {
+#pragma unroll
+        for (int k = 0; k < 2 * ND; ++k) { nb[k] = -1; Lf[k] = (T)0; }
+    }
+    T* cur = XA;
+    T* oth = XB;
+    for (int s = 0; s < sweeps; ++s) {
+        T xn;
+        if (s == 0 && from_zero) {
+            xn = cI * ((T)0 - bI);
+        } else {
+            T a = 0;
+#pragma unroll
+            for (int k = 0; k < 2 * ND; ++k)
+                if (nb[k] >= 0) a += Lf[k] * (cur[nb[k]] - xv);
+            xn = xv + cI * (a - bI);
+        }
+        xv = xn;
+        if (has) oth[I] = xn;
+        bar_sync_n(1, nthr);
+        T* tmp = cur; cur = oth; oth = tmp;
+    }
+    // an even number of sweeps ends with cur == XA
 }
 
 template <typename T, int ND>
@@ -85,7 +170,7 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_coarse_tail(TailParams<T> P
         T* C = CC(l);
         for (int I = threadIdx.x; I < (int)g.M; I += blockDim.x) {
             int i0, i1, i2;
-            decompose<T, ND>(g, I, i0, i1, i2);
+            decompose_i<ND>(g, I, i0, i1, i2);
             const int Ii[3] = {i0, i1, i2};
             const int Ni[3] = {g.N0, g.N1, g.N2};
             const int st[3] = {1, g.N0, g.N0 * g.N1};
@@ -124,23 +209,21 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_coarse_tail(TailParams<T> P
             T* r = XB(l);                                                           // XB is free: fine residual
             for (int I = threadIdx.x; I < (int)gf.M; I += nthr) {
                 int i0, i1, i2;
-                decompose<T, ND>(gf, I, i0, i1, i2);
-                T Ax, D;
-                stencil_cell<T, ND>(gf, L, x, I, i0, i1, i2, Ax, D);
-                r[I] = b[I] - Ax;
+                decompose_i<ND>(gf, I, i0, i1, i2);
+                r[I] = b[I] - stencil_i<T, ND>(gf, L, x, I, i0, i1, i2);
             }
             bar_sync_n(1, nthr);
             T* bc = B(l + 1);
             for (int J = threadIdx.x; J < (int)gc.M; J += nthr) {                   // b_{l+1} = R r: pairwise along 0, 1, 2
                 int j0, j1, j2;
-                decompose<T, ND>(gc, J, j0, j1, j2);
+                decompose_i<ND>(gc, J, j0, j1, j2);
                 T s2[2] = {0, 0};
 #pragma unroll
                 for (int c2 = 0; c2 < (ND == 3 ? 2 : 1); ++c2) {
                     T s1[2];
 #pragma unroll
                     for (int c1 = 0; c1 < 2; ++c1) {
-                        const long long I = cell_index(gf, 2 * j0, 2 * j1 + c1, (ND == 3) ? 2 * j2 + c2 : 0);
+                        const int I = 2 * j0 + gf.N0 * ((2 * j1 + c1) + gf.N1 * ((ND == 3) ? 2 * j2 + c2 : 0));
                         s1[c1] = r[I] + r[I + 1];
                     }
                     s2[c2] = s1[0] + s1[1];
@@ -156,10 +239,14 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_coarse_tail(TailParams<T> P
         const int nthr = nthr_of(last);
         if ((int)threadIdx.x < nthr) {
             const bool zero = (last > 0) ? true : (P.zero_in || P.coarsest_is_correction);
+            if ((int)g.M <= nthr) {
+                tail_sweeps_cached<T, ND>(g, LL(last), CC(last), XA(last), XB(last), B(last), zero, 64, nthr);
+            } else {
             tail_sweep<T, ND>(g, LL(last), CC(last), XA(last), B(last), XB(last), zero, nthr);
             for (int s = 1; s < 64; s += 2) {
                 tail_sweep<T, ND>(g, LL(last), CC(last), XB(last), B(last), XA(last), false, nthr);
                 if (s + 1 < 64) tail_sweep<T, ND>(g, LL(last), CC(last), XA(last), B(last), XB(last), false, nthr);
+            }
             }
         }
     }
@@ -175,8 +262,8 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_coarse_tail(TailParams<T> P
             const T* xc = XA(l + 1);
             for (int I = threadIdx.x; I < (int)gf.M; I += nthr) {
                 int i0, i1, i2;
-                decompose<T, ND>(gf, I, i0, i1, i2);
-                x[I] += xc[cell_index(gc, i0 >> 1, i1 >> 1, i2 >> 1)];
+                decompose_i<ND>(gf, I, i0, i1, i2);
+                x[I] += xc[(i0 >> 1) + gc.N0 * ((i1 >> 1) + gc.N1 * (i2 >> 1))];
             }
             bar_sync_n(1, nthr);
             tail_sweep<T, ND>(gf, LL(l), CC(l), XA(l), B(l), XB(l), false, nthr);
