@@ -29,6 +29,7 @@ constexpr int kTailSmemBudget = 200 * 1024;
 struct Level {
     Grid g;
     void* L = nullptr;      // n*M coefficients (ctx-owned copy / coarsened)
+    void* C = nullptr;      // M: omega / D per cell (0 where D = 0), derived from L by wl_set_coeff
     void* x[2] = {nullptr, nullptr};  // level >= 1: iterate ping-pong; level 0: x[1] = ctx-owned scratch only
     void* b = nullptr;      // level >= 1: restricted residual
     void* tmp = nullptr;    // generic path only: second half of the Jacobi ping-pong (allocated on first use)
@@ -138,6 +139,16 @@ struct Impl {
             k_coarsen<T, ND><<<grid_for(c, b.g.M * ND), kBlock, 0, c->stream>>>(a.g, b.g, P(a.L), P(b.L));
             KCHECK(c, "k_coarsen");
         }
+        for (int l = 0; l < c->nlev; ++l) {   // omega / D per cell, once per coefficient set
+            Level& v = c->lev[l];
+            if (rows_ok(v.g, v.L, v.C)) {
+                k_make_c_rows<T, ND><<<rows_grid(c, (long long)v.g.N1 * v.g.N2), dim3(kRowsX, kRowsY), 0, c->stream>>>(v.g, P(v.L), P(v.C));
+                KCHECK(c, "k_make_c_rows");
+            } else {
+                k_make_c<T, ND><<<grid_for(c, v.g.M), kBlock, 0, c->stream>>>(v.g, P(v.L), P(v.C));
+                KCHECK(c, "k_make_c");
+            }
+        }
         c->have_coeff = true;
         return WL_OK;
     }
@@ -216,7 +227,8 @@ struct Impl {
 
 
     // ---- fused level halves (wl_fused3d.cuh) ---------------------------------------------------------------------
-    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? 16 : 14, FPF = 3;   // 12 warps each
+    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? 16 : 14;   // 12 warps each
+    template <bool PROLONG> static constexpr int FPF = PROLONG ? 2 : 3;   // planes in flight: what fits 227 KB beside the ring
 
     // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
     // vectors; opt_fused == 1 keeps levels smaller than one tile on the generic kernels, 2 forces them (tests).
@@ -284,10 +296,10 @@ struct Impl {
         if constexpr (ND == 3) {
             using G = F3<T, FTX, FTY>;
             Level& f = c->lev[l];
-            CUtensorMap mx, mb, mL0, mL1, mL2, mxc;
+            CUtensorMap mx, mb, mL0, mL1, mL2, mC, mxc;
             bool ok = map_cells(&mb, b, f.g, false);
             ok = ok && map_cells(&mL0, P(f.L), f.g, false) && map_cells(&mL1, P(f.L) + f.g.M, f.g, false) &&
-                 map_cells(&mL2, P(f.L) + 2 * f.g.M, f.g, false);
+                 map_cells(&mL2, P(f.L) + 2 * f.g.M, f.g, false) && map_cells(&mC, P(f.C), f.g, false);
             if (ZERO_IN) mx = mb; else ok = ok && map_cells(&mx, x_in, f.g, false);
             if (PROLONG) ok = ok && map_cells(&mxc, xc, c->lev[l + 1].g, true); else mxc = mb;
             if (!ok) return fail(c, WL_ECUDA, "cuTensorMapEncodeTiled refused a level array (alignment?)");
@@ -313,13 +325,13 @@ struct Impl {
             prm.scal = c->d_scal;
             prm.partials = c->d_partials;
             prm.check_done = c->check_done;
-            auto kern = k_fused3d<T, FTX, FTY, FPF, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN>;
-            constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF, PROLONG>();
+            auto kern = k_fused3d<T, FTX, FTY, FPF<PROLONG>, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN>;
+            constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF<PROLONG>, PROLONG>();
             long long g = ntiles * best_nc;
             if (g > c->num_sms) g = c->num_sms;
             if (NORMS && g > kMaxPartials) g = kMaxPartials;
             c->fused_grid = (int)g;
-            kern<<<(int)g, G::NT, smem, c->stream>>>(mx, mb, mL0, mL1, mL2, mxc, prm);
+            kern<<<(int)g, G::NT, smem, c->stream>>>(mx, mb, mL0, mL1, mL2, mC, mxc, prm);
             KCHECK(c, "k_fused3d");
             return WL_OK;
         } else {
@@ -514,14 +526,14 @@ struct Impl {
     // Set every opt-in shared-memory size once, outside any stream capture.
     static int init_kernels(wl_ctx* c) {
         if constexpr (ND == 3) {
-            constexpr size_t s0 = fused3d_smem_bytes<T, FTX, FTY, FPF, false>(), s1 = fused3d_smem_bytes<T, FTX, FTY, FPF, true>();
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, false, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, false, true, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, true, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, false, false, true, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF, true, false, false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+            constexpr size_t s0 = fused3d_smem_bytes<T, FTX, FTY, FPF<false>, false>(), s1 = fused3d_smem_bytes<T, FTX, FTY, FPF<true>, true>();
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, true, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, true, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
         }
         if constexpr (ND == 2) {
             constexpr int s2 = (int)fused2d_smem_bytes<T, F2TX, F2TY>();
@@ -786,6 +798,7 @@ int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
     for (int l = 0; l < nlev; ++l) {
         Level& v = c->lev[l];
         dmalloc(&v.L, (size_t)v.g.M * ndim * c->esz);
+        dmalloc(&v.C, (size_t)v.g.M * c->esz);
         dmalloc(&v.x[1], (size_t)v.g.M * c->esz);
         if (l > 0) {
             dmalloc(&v.x[0], (size_t)v.g.M * c->esz);
@@ -830,6 +843,7 @@ void wl_destroy(wl_ctx* c) {
     for (int l = 0; l < kMaxLevels; ++l) {
         Level& v = c->lev[l];
         if (v.L) cudaFree(v.L);
+        if (v.C) cudaFree(v.C);
         if (v.x[0]) cudaFree(v.x[0]);
         if (v.x[1]) cudaFree(v.x[1]);
         if (v.b) cudaFree(v.b);

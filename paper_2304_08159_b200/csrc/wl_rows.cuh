@@ -7,6 +7,7 @@
 #pragma once
 #include "wl_common.cuh"
 #include "wl_fused3d.cuh"  // ld_vec / st_vec
+#include "wl_generic.cuh"  // decompose
 
 namespace wl {
 
@@ -134,6 +135,71 @@ __global__ void __launch_bounds__(kRowsX* kRowsY) k_gradient_rows(Grid g, const 
                 st_vec<T, VEC>(u + 2 * g.M + e0, uu);
             }
         }
+    }
+}
+
+// C = omega * invD per cell, D = sum of the cell's 2n face coefficients in the oracle's order ((Lm + Lp) per axis, axes
+// 0, 1, 2), invD = D > 0 ? 1/D : 0 with IEEE division: exactly the factor the oracle forms in every sweep.  Computed
+// once per coefficient set and level; the fused kernels load it instead of recomputing D and a reciprocal per sweep.
+template <typename T, int ND>
+__global__ void __launch_bounds__(kRowsX* kRowsY) k_make_c_rows(Grid g, const T* __restrict__ L, T* __restrict__ C) {
+    constexpr int VEC = 16 / (int)sizeof(T);
+    const int nvx = g.N0 / VEC;
+    const long long nrows = (long long)g.N1 * g.N2;
+    const long long sy = g.N0, sz = (long long)g.N0 * g.N1;
+    const T omega = Omega<T>::value();
+    for (long long r = (long long)blockIdx.x * kRowsY + threadIdx.y; r < nrows; r += (long long)gridDim.x * kRowsY) {
+        const int z = (int)(r / g.N1), y = (int)(r - (long long)z * g.N1);
+        const T* l0 = L + r * g.N0;
+        const T* l1 = l0 + g.M;
+        const T* l2 = l1 + g.M;
+        const bool up1 = (y + 1 < g.N1), up2 = (ND == 3) && (z + 1 < g.N2);
+        for (int vx = threadIdx.x; vx < nvx; vx += kRowsX) {
+            const int x = vx * VEC;
+            T a0[VEC], a1[VEC], a1p[VEC], a2[VEC], a2p[VEC], out[VEC];
+            ld_vec<T, VEC>(l0 + x, a0);
+            const T a0n = (x + VEC < g.N0) ? l0[x + VEC] : (T)0;
+            ld_vec<T, VEC>(l1 + x, a1);
+            if (up1) ld_vec<T, VEC>(l1 + x + sy, a1p);
+            if (ND == 3) {
+                ld_vec<T, VEC>(l2 + x, a2);
+                if (up2) ld_vec<T, VEC>(l2 + x + sz, a2p);
+            }
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) {
+                const T e = (k + 1 < VEC) ? a0[(k + 1) % VEC] : a0n;
+                // wall faces: the stored plane I_i = 0 is already 0 in the library's copy; the unstored upper wall is 0
+                T D = 0;
+                D += a0[k] + e;
+                D += a1[k] + (up1 ? a1p[k] : (T)0);
+                if (ND == 3) D += a2[k] + (up2 ? a2p[k] : (T)0);
+                const T invD = (D > (T)0) ? (T)1 / D : (T)0;
+                out[k] = omega * invD;
+            }
+            st_vec<T, VEC>(C + r * g.N0 + x, out);
+        }
+    }
+}
+// Any-shape version (rows that are not whole vectors).
+template <typename T, int ND>
+__global__ void k_make_c(Grid g, const T* __restrict__ L, T* __restrict__ C) {
+    const T omega = Omega<T>::value();
+    const int Ni[3] = {g.N0, g.N1, g.N2};
+    const long long st[3] = {1, (long long)g.N0, (long long)g.N0 * g.N1};
+    for (long long I = (long long)blockIdx.x * blockDim.x + threadIdx.x; I < g.M; I += (long long)gridDim.x * blockDim.x) {
+        int i0, i1, i2;
+        decompose<T, ND>(g, I, i0, i1, i2);
+        const int Ii[3] = {i0, i1, i2};
+        T D = 0;
+#pragma unroll
+        for (int i = 0; i < ND; ++i) {
+            const T* Li = L + (long long)i * g.M;
+            const T Lp = (Ii[i] + 1 < Ni[i]) ? Li[I + st[i]] : (T)0;
+            const T Lm = (Ii[i] > 0) ? Li[I] : (T)0;
+            D += Lm + Lp;
+        }
+        const T invD = (D > (T)0) ? (T)1 / D : (T)0;
+        C[I] = omega * invD;
     }
 }
 
