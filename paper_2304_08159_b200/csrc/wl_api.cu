@@ -549,16 +549,21 @@ struct Impl {
         return WL_OK;
     }
 
-    static int divergence(wl_ctx* c, const void* u, void* b) {
+    // with_nb: also leave ||b||inf in slot 0 (fused into the row kernel; one more pass on the generic path)
+    static int divergence(wl_ctx* c, const void* u, void* b, bool with_nb) {
         Level& f = c->lev[0];
         if (rows_ok(f.g, u, b)) {
-            k_divergence_rows<T, ND><<<rows_grid(c, (long long)f.g.N1 * f.g.N2), dim3(kRowsX, kRowsY), 0, c->stream>>>(f.g, P(u), P(b));
+            if (with_nb) {
+                k_zero_slot<<<1, 32, 0, c->stream>>>(c->d_scal, 0);
+                KCHECK(c, "k_zero_slot");
+            }
+            k_divergence_rows<T, ND><<<rows_grid(c, (long long)f.g.N1 * f.g.N2), dim3(kRowsX, kRowsY), 0, c->stream>>>(f.g, P(u), P(b), with_nb ? c->d_scal : nullptr);
             KCHECK(c, "k_divergence_rows");
             return WL_OK;
         }
         k_divergence<T, ND><<<grid_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, P(u), P(b));
         KCHECK(c, "k_divergence");
-        return WL_OK;
+        return with_nb ? absmax_b(c, b) : WL_OK;
     }
 
     static int gradient(wl_ctx* c, void* u, const void* p) {
@@ -683,47 +688,63 @@ int wait_cycle(wl_ctx* c, int target) {
     }
 }
 
-int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, double* hist, int* ncycles) {
+// have_nb: ||b||inf is already in slot 0 (wl_project's divergence kernel left it there).
+int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, double* hist, int* ncycles, bool have_nb = false) {
     int rc;
     if ((rc = ensure_hist(c, maxcycles))) return rc;
-    if ((rc = DISPATCH(c, absmax_b)(c, b))) return rc;
-    if ((rc = DISPATCH(c, resnorm)(c, p, b))) return rc;
-    k_solve_begin<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, tol, maxcycles);
-    KCHECK(c, "k_solve_begin");
-    if ((rc = read_scalars(c))) return rc;
-    const double nb = c->h_scal->nb;
-    hist[0] = bits_to_double(c->h_scal->absmax_bits[1]);
-    const bool deferred = DISPATCH(c, can_defer)(c) && DISPATCH(c, can_speculate)(c);
-    // Cycles are enqueued up to `depth` ahead of the stop test; the host polls the pinned mirror k_cycle_end writes
-    // instead of synchronising the stream, so the GPU does not idle for a host round trip per cycle.
+    if (!have_nb && (rc = DISPATCH(c, absmax_b)(c, b))) return rc;
     const bool spec = DISPATCH(c, can_speculate)(c);
-    const bool lagged = deferred && spec;   // hist[k] is read off the DOWN kernel of launch k+1 (k_cycle_check)
-    const int depth = spec ? 2 : 1;
+    const bool lagged = spec && DISPATCH(c, can_defer)(c);
     volatile Scalars* hm = c->h_scal;
-    hm->cycle = 0;
-    int launched = 0, k = 0;
-    bool stop = !(maxcycles > 0 && hist[0] > tol * nb);
-    while (!stop) {
-        if (lagged) {
-            while (launched < k + 2 && launched < maxcycles + 1) {
+    double nb = 0.0;
+    int k = 0;
+    if (lagged) {
+        // Lagged stop test: launch g's level-0 DOWN kernel measures ||b - A p_{g-1}||inf (g = 1: the
+        // initial residual) and k_cycle_check decides on the device; two launches stay enqueued, the host polls the
+        // pinned mirror instead of synchronising, so the GPU never waits for a host round trip.
+        CU(c, cudaStreamSynchronize(c->stream));   // nothing of an earlier call may still write the mirror
+        hm->cycle = 0;
+        k_solve_begin_lagged<<<1, 32, 0, c->stream>>>(c->d_scal, tol, maxcycles);
+        KCHECK(c, "k_solve_begin_lagged");
+        int launched = 0, known = 0;
+        while (true) {
+            while (launched < known + 2 && launched < maxcycles + 1) {
                 if ((rc = run_cycle(c, p, b, true, true, true))) return rc;
                 ++launched;
             }
+            if ((rc = wait_cycle(c, known + 1))) return rc;
+            hist[known] = c->h_hist[known];
+            nb = hm->nb;
+            k = known++;
+            if (!(hist[k] > tol * nb) || k >= maxcycles) break;
+        }
+        if (k == 0) {
+            if ((rc = DISPATCH(c, remove_mean)(c, p))) return rc;
         } else {
+            if ((rc = DISPATCH(c, apply_shift)(c, p))) return rc;
+        }
+    } else {
+        if ((rc = DISPATCH(c, resnorm)(c, p, b))) return rc;
+        k_solve_begin<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, tol, maxcycles);
+        KCHECK(c, "k_solve_begin");
+        if ((rc = read_scalars(c))) return rc;
+        nb = c->h_scal->nb;
+        hist[0] = bits_to_double(c->h_scal->absmax_bits[1]);
+        const int depth = spec ? 2 : 1;
+        hm->cycle = 0;
+        int launched = 0;
+        bool stop = !(maxcycles > 0 && hist[0] > tol * nb);
+        while (!stop) {
             while (launched < maxcycles && launched - k < depth) {
-                if ((rc = run_cycle(c, p, b, deferred, true))) return rc;
+                if ((rc = run_cycle(c, p, b, false, true))) return rc;
                 ++launched;
             }
+            if ((rc = wait_cycle(c, k + 1))) return rc;
+            ++k;
+            hist[k] = c->h_hist[k];
+            if (!(hist[k] > tol * nb) || k >= maxcycles) stop = true;
         }
-        if ((rc = wait_cycle(c, k + 1))) return rc;
-        ++k;
-        hist[k] = c->h_hist[k];
-        if (!(hist[k] > tol * nb) || k >= maxcycles) stop = true;
-    }
-    if (k == 0) {
-        if ((rc = DISPATCH(c, remove_mean)(c, p))) return rc;
-    } else if (deferred) {
-        if ((rc = DISPATCH(c, apply_shift)(c, p))) return rc;
+        if (k == 0 && (rc = DISPATCH(c, remove_mean)(c, p))) return rc;
     }
     CU(c, cudaStreamSynchronize(c->stream));
     *ncycles = k;
@@ -915,8 +936,8 @@ int wl_project(wl_ctx* c, void* u, const void* L, void* p, double tol, int maxcy
     if (!c->b0) {
         if (cudaMalloc(&c->b0, (size_t)c->lev[0].g.M * c->esz) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "wl_project: cudaMalloc(b)"); }
     }
-    if ((rc = DISPATCH(c, divergence)(c, u, c->b0))) return rc;
-    int src = solve_impl(c, p, c->b0, tol, maxcycles, hist, ncycles);
+    if ((rc = DISPATCH(c, divergence)(c, u, c->b0, true))) return rc;
+    int src = solve_impl(c, p, c->b0, tol, maxcycles, hist, ncycles, true);
     if (src < 0) return src;
     if ((rc = DISPATCH(c, gradient)(c, u, p))) return rc;
     CU(c, cudaStreamSynchronize(c->stream));
@@ -946,7 +967,7 @@ int wl_project_host(wl_ctx* c, void* u_host, const void* L_host, void* p_host, d
 int wl_divergence(wl_ctx* c, const void* u, void* b) {
     if (!c) return WL_EINVAL;
     if (!u || !b) return fail(c, WL_EINVAL, "wl_divergence: null pointer");
-    return DISPATCH(c, divergence)(c, u, b);
+    return DISPATCH(c, divergence)(c, u, b, false);
 }
 
 int wl_gradient(wl_ctx* c, void* u, const void* p) {

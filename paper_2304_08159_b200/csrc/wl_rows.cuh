@@ -43,11 +43,13 @@ __global__ void __launch_bounds__(kRowsX* kRowsY) k_copy_coeff_rows(Grid g, cons
 
 // H1: b[I] = sum_i (u[i][I+d_i] - u[i][I]), unstored upper wall face = 0.
 template <typename T, int ND>
-__global__ void __launch_bounds__(kRowsX* kRowsY) k_divergence_rows(Grid g, const T* __restrict__ u, T* __restrict__ b) {
+__global__ void __launch_bounds__(kRowsX* kRowsY) k_divergence_rows(Grid g, const T* __restrict__ u, T* __restrict__ b,
+                                                                   Scalars* scal /* nullable: ||b||inf -> slot 0 */) {
     constexpr int VEC = 16 / (int)sizeof(T);
     const int nvx = g.N0 / VEC;
     const long long nrows = (long long)g.N1 * g.N2;
     const long long sy = g.N0, sz = (long long)g.N0 * g.N1;
+    T bmax = (T)0;
     for (long long r = (long long)blockIdx.x * kRowsY + threadIdx.y; r < nrows; r += (long long)gridDim.x * kRowsY) {
         const int z = (int)(r / g.N1), y = (int)(r - (long long)z * g.N1);
         const T* u0 = u + r * g.N0;
@@ -82,8 +84,21 @@ __global__ void __launch_bounds__(kRowsX* kRowsY) k_divergence_rows(Grid g, cons
                 s += a1p[k] - a1[k];
                 if (ND == 3) s += a2p[k] - a2[k];
                 out[k] = s;
+                bmax = fmax(bmax, fabs(s));
             }
             st_vec<T, VEC>(b + r * g.N0 + x, out);
+        }
+    }
+    if (scal) {   // uniform branch: every thread of the CTA takes it
+        __shared__ double red[32];
+        double m = warp_max((double)bmax);
+        const int tid = threadIdx.y * kRowsX + threadIdx.x;
+        if ((tid & 31) == 0) red[tid >> 5] = m;
+        __syncthreads();
+        if (tid < 32) {
+            m = (tid < (kRowsX * kRowsY) / 32) ? red[tid] : 0.0;
+            m = warp_max(m);
+            if (tid == 0) atomic_max_nonneg(&scal->absmax_bits[0], m);
         }
     }
 }
