@@ -340,30 +340,17 @@ struct Impl {
     }
 
     // DOWN half of level l: x_out = J(J(x_in)) (x_in == nullptr: from zero), bc = R(b - A x_out).
-    static int down(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out, void* bc, bool shift = false) {
-        if (!fused_ok(c, l)) return shift ? fail(c, WL_EINVAL, "deferred mean shift needs the fused level-0 kernel") : down_generic(c, l, x_in, b, x_out, bc);
-        if (x_in && shift) return launch_fused<false, false, true, true, true, false>(c, l, x_in, nullptr, b, x_out, bc);
+    static int down(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out, void* bc) {
+        if (!fused_ok(c, l)) return down_generic(c, l, x_in, b, x_out, bc);
         if (x_in) return launch_fused<false, false, false, true, true, false>(c, l, x_in, nullptr, b, x_out, bc);
         return launch_fused<false, true, false, true, true, false>(c, l, nullptr, nullptr, b, x_out, bc);
     }
 
-    // UP half of level l: x_out = J(J(x_in + P xc)); `norms` (level 0): also ||b - A x_out||inf -> slot 1, sum -> mean.
-    static int up(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out, bool norms) {
-        if (!fused_ok(c, l)) {
-            int rc = up_generic(c, l, x_in, xc, b, x_out);
-            if (rc || !norms) return rc;
-            return resnorm(c, x_out, b);
-        }
-        if (!norms) return launch_fused<true, false, false, false, false, false>(c, l, x_in, xc, b, x_out, nullptr);
-        k_zero_slot<<<1, 32, 0, c->stream>>>(c->d_scal, 1);
-        KCHECK(c, "k_zero_slot");
-        int rc = launch_fused<true, false, false, true, false, true>(c, l, x_in, xc, b, x_out, nullptr);
-        if (rc) return rc;
-        k_finish_mean<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_partials, c->fused_grid, c->lev[0].g.M);
-        KCHECK(c, "k_finish_mean");
-        return WL_OK;
+    // UP half of level l: x_out = J(J(x_in + P xc)).
+    static int up(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out) {
+        if (!fused_ok(c, l)) return up_generic(c, l, x_in, xc, b, x_out);
+        return launch_fused<true, false, false, false, false, false>(c, l, x_in, xc, b, x_out, nullptr);
     }
-
 
     // VCYCLE(l) for a level inside the coarse tail: one persistent CTA (wl_tail.cuh).  x_in == nullptr: zero guess.
     static int tail(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out) {
@@ -411,22 +398,16 @@ struct Impl {
     }
 
     // VCYCLE(l): x_out = cycle(x_in) on level l; x_mid = level-sized scratch (may not alias x_in / x_out).
-    // x_in == nullptr means a zero initial guess (every correction level).  norms: level-0 reductions after the UP half.
-    static int vcycle(wl_ctx* c, int l, const void* x_in, const void* b, void* x_mid, void* x_out, bool norms, bool shift = false) {
+    // x_in == nullptr means a zero initial guess (every correction level).
+    static int vcycle(wl_ctx* c, int l, const void* x_in, const void* b, void* x_mid, void* x_out) {
         int rc;
-        if (c->opt_coarse_cta && l >= c->tail_first) {
-            const void* xi = (l == c->nlev - 1 && l > 0) ? nullptr : x_in;
-            if ((rc = tail(c, l, xi, b, x_out))) return rc;
-            return norms ? resnorm(c, x_out, b) : WL_OK;
-        }
-        if (l == c->nlev - 1) {
-            if ((rc = coarsest(c, l, (c->nlev > 1 && l > 0) ? nullptr : x_in, b, x_mid, x_out))) return rc;
-            return norms ? resnorm(c, x_out, b) : WL_OK;
-        }
+        if (c->opt_coarse_cta && l >= c->tail_first)
+            return tail(c, l, (l == c->nlev - 1 && l > 0) ? nullptr : x_in, b, x_out);
+        if (l == c->nlev - 1) return coarsest(c, l, (c->nlev > 1 && l > 0) ? nullptr : x_in, b, x_mid, x_out);
         Level& k = c->lev[l + 1];
-        if ((rc = down(c, l, x_in, b, x_mid, k.b, shift))) return rc;
-        if ((rc = vcycle(c, l + 1, nullptr, k.b, k.x[0], k.x[1], false))) return rc;
-        return up(c, l, x_mid, k.x[1], b, x_out, norms);
+        if ((rc = down(c, l, x_in, b, x_mid, k.b))) return rc;
+        if ((rc = vcycle(c, l + 1, nullptr, k.b, k.x[0], k.x[1]))) return rc;
+        return up(c, l, x_mid, k.x[1], b, x_out);
     }
 
     // Σp -> mean (ordered), p -= mean.
@@ -485,14 +466,11 @@ struct Impl {
         return WL_OK;
     }
 
-    // One V-cycle; ||b - A p||inf (slot 1) and mean(p) come out of the level-0 UP half.  The norm is taken before the
-    // shift: A·1 = 0, so it differs from the oracle's (after the shift) by rounding only.
-    // deferred: p enters unshifted (scal->shift pending) and leaves unshifted; k_cycle_end moves mean -> shift.
-    static int cycle(wl_ctx* c, void* p, const void* b, bool deferred) {
+    // One V-cycle in the oracle's literal order: VCYCLE(0), p -= mean(p), ||b - A p||inf of the shifted p (slot 1).
+    // Used by wl_vcycle and by solves whose level 0 is not fused; the fused solve uses cycle_lagged.
+    static int cycle(wl_ctx* c, void* p, const void* b) {
         int rc;
-        if (deferred) return vcycle(c, 0, p, b, c->lev[0].x[1], p, true, true);
-        // classic order, exactly the oracle's: V-cycle, p -= mean(p), then ||b - A p||inf of the shifted p
-        if ((rc = vcycle(c, 0, p, b, c->lev[0].x[1], p, false, false))) return rc;
+        if ((rc = vcycle(c, 0, p, b, c->lev[0].x[1], p))) return rc;
         if ((rc = remove_mean(c, p))) return rc;
         return resnorm(c, p, b);
     }
@@ -514,7 +492,7 @@ struct Impl {
         if ((rc = launch_fused<false, false, true, true, true, false, true>(c, 0, p, nullptr, b, c->lev[0].x[1], k1.b))) return rc;
         k_cycle_check<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, c->h_scal, c->h_hist);
         KCHECK(c, "k_cycle_check");
-        if ((rc = vcycle(c, 1, nullptr, k1.b, k1.x[0], k1.x[1], false, false))) return rc;
+        if ((rc = vcycle(c, 1, nullptr, k1.b, k1.x[0], k1.x[1]))) return rc;
         if ((rc = launch_fused<true, false, false, false, false, true, false>(c, 0, c->lev[0].x[1], k1.x[1], b, p, nullptr))) return rc;
         k_finish_mean<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_partials, c->fused_grid, c->lev[0].g.M);
         KCHECK(c, "k_finish_mean");
@@ -528,20 +506,16 @@ struct Impl {
         if constexpr (ND == 3) {
             constexpr size_t s0 = fused3d_smem_bytes<T, FTX, FTY, FPF<false>, false>(), s1 = fused3d_smem_bytes<T, FTX, FTY, FPF<true>, true>();
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, true, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, true, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
         }
         if constexpr (ND == 2) {
             constexpr int s2 = (int)fused2d_smem_bytes<T, F2TX, F2TY>();
             CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
-            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, true, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
             CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
             CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
-            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
             CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, true, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
             CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
         }
@@ -617,17 +591,17 @@ void drop_graph(wl_ctx* c) {
 }
 
 // One V-cycle (+ k_cycle_end bookkeeping when `in_solve`) on the ctx stream: a cached CUDA graph when WL_OPT_GRAPH is on.
-// variant: bit 0 = deferred mean shift, bit 1 = in_solve.
-int run_cycle(wl_ctx* c, void* p, const void* b, bool deferred, bool in_solve, bool lagged = false) {
+// variant: bit 0 = in_solve, bit 1 = lagged.
+int run_cycle(wl_ctx* c, void* p, const void* b, bool in_solve, bool lagged) {
     int rc;
-    const int variant = (deferred ? 1 : 0) | (in_solve ? 2 : 0) | (lagged ? 4 : 0);
+    const int variant = (in_solve ? 1 : 0) | (lagged ? 2 : 0);
     auto enqueue = [&]() -> int {
         c->check_done = in_solve ? 1 : 0;
-        int r = lagged ? DISPATCH(c, cycle_lagged)(c, p, b) : DISPATCH(c, cycle)(c, p, b, deferred);
+        int r = lagged ? DISPATCH(c, cycle_lagged)(c, p, b) : DISPATCH(c, cycle)(c, p, b);
         c->check_done = 0;
         if (r) return r;
         if (in_solve && !lagged) {
-            k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, deferred ? 1 : 0, c->h_scal, c->h_hist);
+            k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, 0, c->h_scal, c->h_hist);
             KCHECK(c, "k_cycle_end");
         }
         return WL_OK;
@@ -709,7 +683,7 @@ int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, dou
         int launched = 0, known = 0;
         while (true) {
             while (launched < known + 2 && launched < maxcycles + 1) {
-                if ((rc = run_cycle(c, p, b, true, true, true))) return rc;
+                if ((rc = run_cycle(c, p, b, true, true))) return rc;
                 ++launched;
             }
             if ((rc = wait_cycle(c, known + 1))) return rc;
@@ -736,7 +710,7 @@ int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, dou
         bool stop = !(maxcycles > 0 && hist[0] > tol * nb);
         while (!stop) {
             while (launched < maxcycles && launched - k < depth) {
-                if ((rc = run_cycle(c, p, b, false, true))) return rc;
+                if ((rc = run_cycle(c, p, b, true, false))) return rc;
                 ++launched;
             }
             if ((rc = wait_cycle(c, k + 1))) return rc;
@@ -1001,21 +975,21 @@ int wl_down(wl_ctx* c, int level, const void* x_in, const void* b, void* x_out, 
     if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_down: bad level") : WL_EINVAL;
     if (!b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_down: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_down: coefficients not set");
-    return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b, false);
+    return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
 }
 
 int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b, void* x_out) {
     if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_up: bad level") : WL_EINVAL;
     if (!x_in || !b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_up: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_up: coefficients not set");
-    return DISPATCH(c, up)(c, level, x_in, xc ? xc : c->lev[level + 1].x[1], b, x_out, false);
+    return DISPATCH(c, up)(c, level, x_in, xc ? xc : c->lev[level + 1].x[1], b, x_out);
 }
 
 int wl_vcycle_level(wl_ctx* c, int level, void* x, const void* b) {
     if (level_check(c, level, false)) return c ? fail(c, WL_EINVAL, "wl_vcycle_level: bad level") : WL_EINVAL;
     if (!x || !b) return fail(c, WL_EINVAL, "wl_vcycle_level: null pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle_level: coefficients not set");
-    return DISPATCH(c, vcycle)(c, level, x, b, level == 0 ? c->lev[0].x[1] : c->lev[level].x[0], x, false, false);
+    return DISPATCH(c, vcycle)(c, level, x, b, level == 0 ? c->lev[0].x[1] : c->lev[level].x[0], x);
 }
 
 int wl_residual_norm(wl_ctx* c, const void* p, const void* b, double* rnorm_out, double* mean_out) {
