@@ -228,7 +228,7 @@ struct Impl {
 
     // ---- fused level halves (wl_fused3d.cuh) ---------------------------------------------------------------------
     static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? 16 : 14;   // 12 warps each
-    template <bool PROLONG> static constexpr int FPF = PROLONG ? 2 : 3;   // planes in flight: what fits 227 KB beside the ring
+    template <bool PROLONG> static constexpr int FPF = (PROLONG && WL_UP_LOADS_C) ? 2 : 3;   // planes in flight: what fits 227 KB beside the ring
 
     // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
     // vectors; opt_fused == 1 keeps levels smaller than one tile on the generic kernels, 2 forces them (tests).
