@@ -36,10 +36,12 @@ __device__ __forceinline__ void bar_sync_n(int id, int nthreads) {
 // 32-bit index helpers (tail levels have at most a few thousand cells): no 64-bit divisions in the sweeps.
 template <int ND>
 __device__ __forceinline__ void decompose_i(const Grid& g, int I, int& i0, int& i1, int& i2) {
-    const int q = I / g.N0;
+    // exact for the tail's sizes (I < 2^16, N < 2^10): the float quotient of (I + 1/2) / N is never within rounding
+    // error of an integer
+    const int q = __float2int_rz(((float)I + 0.5f) * __frcp_rn((float)g.N0));
     i0 = I - q * g.N0;
     if (ND == 3) {
-        const int q2 = q / g.N1;
+        const int q2 = __float2int_rz(((float)q + 0.5f) * __frcp_rn((float)g.N1));
         i1 = q - q2 * g.N1;
         i2 = q2;
     } else {
