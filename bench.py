@@ -135,7 +135,7 @@ def run_reference(args, rank: int):
     from paper_2304_08159_b200 import synth
     import oracle
     oracle.build()
-    cfg = synth.make_config(args.config, scale=args.scale)
+    cfg = synth.make_donut(args.donut) if args.donut else synth.make_config(args.config, scale=args.scale)
     dims, dt = cfg["dims"], cfg["dtype"]
     M = int(np.prod(dims))
     o = oracle.Oracle(dims, dt)
@@ -171,6 +171,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--scale", type=int, default=1, help="divide every extent (debug only; the default 1 is the workload)")
+    ap.add_argument("--donut", type=int, default=0, help="P in 4..7: the paper-shaped (2^(P+1), 2^P, 2^P) torus grid instead of --config")
     ap.add_argument("--dtype", default=None, choices=[None, "float32", "float64"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -205,7 +206,7 @@ def main():
         torch.cuda.synchronize()
 
     dt_np = None if args.dtype is None else np.dtype(args.dtype)
-    cfg = synth.make_config(args.config, dtype=dt_np, scale=args.scale)
+    cfg = synth.make_donut(args.donut, dtype=dt_np) if args.donut else synth.make_config(args.config, dtype=dt_np, scale=args.scale)
     dims, dt = cfg["dims"], cfg["dtype"]
     n, M, esz = len(dims), int(np.prod(dims)), cfg["dtype"].itemsize
     tol, maxc = cfg["tol"], cfg["maxcycles"]
@@ -313,7 +314,7 @@ def main():
         ach = bytes_down / (kern["down"]["ms"] * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": "level-0 DOWN (2 pre-sweeps + residual + restriction), via wl_down",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": NCU_TRAFFIC_DOWN_512 if (args.config == 4 and args.scale == 1 and dt == np.float32) else None,
+                "traffic": NCU_TRAFFIC_DOWN_512 if (args.config == 4 and args.scale == 1 and not args.donut and dt == np.float32) else None,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_down,
                 "launches_per_call": kern["down"]["launches_per_call"], "ms": kern["down"]["ms"],
                 "up_kernel": {"ms": kern["up"]["ms"], "achieved": bytes_down / (kern["up"]["ms"] * 1e-3) / 1e9,

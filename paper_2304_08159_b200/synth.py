@@ -184,6 +184,20 @@ def coeff_spheres(dims, centres, radii, dtype=np.float32, brute_force: bool = Fa
     return zero_walls(L)
 
 
+def coeff_torus(dims, centre, R: float, r: float, dtype=np.float32) -> np.ndarray:
+    """``L = mu0(d)`` for a torus whose axis is the flow axis 0: major radius ``R`` (in the 1-2 plane), minor radius
+    ``r``, ``d = sqrt((sqrt(y^2 + z^2) - R)^2 + x^2) - r`` about ``centre``; face centres, fp64, walls zeroed."""
+    assert len(dims) == 3
+    L = np.empty((3,) + _np_shape(dims), dtype=dtype)
+    for i in range(3):
+        ax = face_axes(dims, i)
+        x, y, z = (ax[j] - float(centre[j]) for j in range(3))
+        rho = np.sqrt(y * y + z * z) - float(R)
+        d = np.sqrt(rho * rho + x * x) - float(r)
+        L[i] = mu0(d).astype(dtype)
+    return zero_walls(L)
+
+
 # ------------------------------------------------------------------------------------------------
 # velocity fields
 # ------------------------------------------------------------------------------------------------
@@ -287,3 +301,18 @@ def make_config(config: int, dtype=None, scale: int = 1) -> dict:
     u *= L  # BDIM-masked velocity (stationary body); walls get u = 0
     return dict(config=config, name=CONFIG_NAMES[config] + (f"_div{s}" if s != 1 else ""),
                 dims=dims, dtype=dt, L=L, u=u, tol=tol, maxcycles=maxc, call=call)
+
+
+def make_donut(p: int, dtype=None) -> dict:
+    """The paper's second workload shape ("flow past a donut ... N = (2^(p+1), 2^p, 2^p)", p = 4..7):
+    a torus in a 2:1:1 box.  The paper gives neither radii nor position; chosen here (and stated in DESIGN.md §5):
+    centre (2^p, 2^(p-1), 2^(p-1)) = the box centre, major radius 2^p / 4, minor radius 2^p / 16 cells, axis along
+    the long (flow) axis.  Velocity as in config 0 (seeded U(-1,1) per face, masked by L); wl_project to 1e-4."""
+    dt = np.dtype(np.float32 if dtype is None else dtype)
+    n1 = 1 << int(p)
+    dims = (2 * n1, n1, n1)
+    L = coeff_torus(dims, (n1, n1 / 2, n1 / 2), n1 / 4.0, n1 / 16.0, dt)
+    u = velocity_uniform(dims, seed_for(5, int(p)), dt)
+    u *= L
+    return dict(config=5, name=f"donut_p{int(p)}_{dims[0]}x{dims[1]}x{dims[2]}", dims=dims, dtype=dt, L=L, u=u,
+                tol=1e-4, maxcycles=32, call="project")

@@ -86,3 +86,20 @@ def test_configs_shapes_and_masks():
     cen, rad = synth.sphere_params(4, (512, 512, 512))
     assert cen.shape == (32, 3) and rad.min() >= 8 and rad.max() <= 32
     assert cen.min() >= 32 and cen.max() <= 480
+
+
+def test_donut_shape_and_coefficients():
+    """Paper-shaped grid: 2:1:1 box, torus about the box centre; L = 0 deep inside the tube, 1 far away,
+    symmetric under reflection of the transverse axes about the centre plane (cell-centred reflection)."""
+    from paper_2304_08159_b200 import synth
+    cfg = synth.make_donut(5)
+    assert cfg["dims"] == (64, 32, 32) and cfg["L"].shape == (3, 32, 32, 64)
+    L = cfg["L"].astype(np.float64)
+    assert L.min() == 0.0 and L.max() == 1.0
+    # a cell centre on the tube's centre circle: x = 32, y = 16 + 8, z = 16 -> faces around it are inside (r = 2)
+    assert L[1, 16, 24, 32] == 0.0 and L[2, 16, 24, 32] == 0.0
+    assert L[0, 2, 2, 5] == 1.0                                   # far corner: fluid
+    assert np.all(L[0, :, :, 0] == 0) and np.all(L[1, :, 0, :] == 0) and np.all(L[2, 0, :, :] == 0)   # walls
+    # component 0 (faces normal to the axis) is symmetric under z -> N2-1-z and y -> N1-1-y (cell-centred in y, z)
+    assert np.array_equal(L[0], L[0][::-1, :, :]) and np.array_equal(L[0], L[0][:, ::-1, :])
+    assert np.array_equal(cfg["u"], (synth.velocity_uniform(cfg["dims"], synth.seed_for(5, 5)) * cfg["L"]))
