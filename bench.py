@@ -69,7 +69,7 @@ def whole_job_value(world: int, cells: int, cycles: int, seconds_per_step: float
 
 
 # DRAM traffic of one level-0 DOWN launch at 512^3 fp32 from the last `ncu --set full` capture (profiles/): bytes.
-NCU_TRAFFIC_DOWN_512 = 3.964e9   # profiles/r1_fused_ncu.md (launch list v14): 3.376 GB read + 0.588 GB written
+NCU_TRAFFIC_DOWN_512 = 3.959e9   # profiles/r1_fused_ncu.md (capture r1_fused_v16_c4): 3.367 GB read + 0.591 GB written
 
 
 class ClockSampler:
