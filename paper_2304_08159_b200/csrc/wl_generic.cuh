@@ -282,13 +282,19 @@ __global__ void k_fill_zero(long long M, T* __restrict__ p) {
 
 // ---- single-thread bookkeeping kernels (ordered second stage of the reductions, stop test) ------------------------
 
-// mean_p = (ordered sum of the per-CTA partials) / M
+// mean_p = (sum of the per-CTA partials in a FIXED order) / M.  One warp: lane l adds partials l, l+32, ... in sequence,
+// then a shuffle tree combines the 32 lane sums — the same order on every run (bit-reproducible), 32 independent
+// chains instead of one serial chain of global loads.
 __global__ void k_finish_mean(Scalars* scal, const double* __restrict__ partials, int nparts, long long M) {
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
+    if (blockIdx.x == 0 && threadIdx.x < 32) {
         double s = 0.0;
-        for (int i = 0; i < nparts; ++i) s += partials[i];
-        scal->sum_p = s;
-        scal->mean_p = s / (double)M;
+        for (int i = threadIdx.x; i < nparts; i += 32) s += partials[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+        if (threadIdx.x == 0) {
+            scal->sum_p = s;
+            scal->mean_p = s / (double)M;
+        }
     }
 }
 
