@@ -17,7 +17,9 @@ The JSON line (rank 0):
              b_c = (n+3+1/2^n)·s per cell) / duration, against MEASURED_PEAKS.json ``hbm_gbs``;
   cpu_baseline  the oracle as it stands on the box's host cores (1 thread), on a bounded sample (one V-cycle of the same
              workload);
-  extra keys: ms per projection, ms per V-cycle (graph launches alone), effective GB/s per V-cycle (56 B/cell model).
+  extra keys: ms per projection, ms per V-cycle (wl_solve with tol = 0 over --kernel-reps cycles: one graph launch per
+             cycle, stop test on the device), effective GB/s per V-cycle (56 B/cell model); roofline.traffic = DRAM bytes of
+             one DOWN launch from the last ncu capture under profiles/ (a recorded constant, ncu never runs here).
 
 N > 1 (torchrun): "replicas only" — every rank projects its own copy of the grid, no collective on the data path
 (BASELINE.json north_star: one GPU, no sharding); value = units all ranks processed / max-over-ranks time.
