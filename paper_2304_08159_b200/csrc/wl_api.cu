@@ -227,8 +227,15 @@ struct Impl {
 
 
     // ---- fused level halves (wl_fused3d.cuh) ---------------------------------------------------------------------
-    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? 16 : 14;   // 12 warps each
-    template <bool PROLONG> static constexpr int FPF = (PROLONG && WL_UP_LOADS_C) ? 2 : 3;   // planes in flight: what fits 227 KB beside the ring
+// Tile height / planes in flight of the fp32 3-D kernels (A/B switches).  Measured at 512^3: TY = 24 with 16 warps
+// (128 registers, 1 plane in flight) runs the DOWN kernel in 0.871 ms against 0.777 ms for TY = 16 with 12 warps.
+#ifndef WL_FTY32
+#define WL_FTY32 16
+#define WL_FPF_DOWN 3
+#define WL_FPF_UP 2
+#endif
+    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? WL_FTY32 : 14;   // 12 warps each
+    template <bool PROLONG> static constexpr int FPF = (PROLONG && WL_UP_LOADS_C) ? WL_FPF_UP : WL_FPF_DOWN;   // planes in flight: what fits 227 KB beside the ring
 
     // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
     // vectors; opt_fused == 1 keeps levels smaller than one tile on the generic kernels, 2 forces them (tests).
