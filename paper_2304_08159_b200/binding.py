@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("WL_LIBRARY") or os.path.join(_HERE, "libwl.so")   # WL_LIBRARY: A/B a differently built libwl
+LIB_PATH = os.path.join(_HERE, "libwl.so")
 
 WL_F32, WL_F64 = 0, 1
 WL_OK, WL_NOT_CONVERGED = 0, 1

@@ -274,12 +274,6 @@ __global__ void k_shift(long long M, T* __restrict__ p, const Scalars* __restric
         p[I] -= m;
 }
 
-template <typename T>
-__global__ void k_fill_zero(long long M, T* __restrict__ p) {
-    for (long long I = (long long)blockIdx.x * blockDim.x + threadIdx.x; I < M; I += (long long)gridDim.x * blockDim.x)
-        p[I] = (T)0;
-}
-
 // ---- single-thread bookkeeping kernels (ordered second stage of the reductions, stop test) ------------------------
 
 // mean_p = (sum of the per-CTA partials in a FIXED order) / M.  One warp: lane l adds partials l, l+32, ... in sequence,

@@ -166,3 +166,55 @@ def test_project_leaves_zero_divergence(oracle_mod, config, scale):
     assert np.abs(div_after - r).max() <= 2e-5 * np.abs(b).max()
     assert abs(p.astype(np.float64).mean()) <= 1e-6 * np.abs(p).max()
     assert np.all(np.diff(hist) < 0)
+
+
+def dense_solve_count(As, Rs, p, b, tol, maxcycles, ref):
+    """The SOLVE loop of BJ "V-cycles repeat until ||r||inf <= tol·||b||inf or 32 cycles" restated with the dense recursion:
+    `ref` is the norm the tolerance multiplies.  Returns (cycles, history)."""
+    hist = [np.abs(b - As[0] @ p).max()]
+    k = 0
+    while k < maxcycles and hist[k] > tol * ref:
+        p = dense_vcycle(As, Rs, 0, p, b)
+        p = p - p.mean()
+        k += 1
+        hist.append(np.abs(b - As[0] @ p).max())
+    return k, np.array(hist)
+
+
+@pytest.mark.parametrize("dims,far", [((16, 16), False), ((16, 16), True), ((8, 8, 8), False), ((8, 8, 8), True)])
+def test_stop_rule_reference_is_norm_of_b_not_initial_residual(oracle_mod, dims, far):
+    """Pins WHICH norm the stop rule multiplies (BJ "until ||r||inf <= 1e-4·||b||inf"): a warm start p0 != 0 with
+    b != 0 makes ||b||inf and the initial residual ||b - A p0||inf differ by orders of magnitude, so the two readings stop
+    after different cycle counts.  The expected count comes from the dense-matrix recursion above, not from the oracle.
+    near: p0 = a partially converged iterate (residual << ||b||): tol·||b|| is met after few (or zero) cycles, tol·hist[0]
+    would need many more.  far: p0 = large noise (residual >> ||b||): tol·hist[0] would stop early, tol·||b|| must not."""
+    rng = np.random.default_rng(300 + dims[0] + len(dims) + (7 if far else 0))
+    n = len(dims)
+    L = random_coeff(dims, rng)
+    As, Rs = dense_hierarchy(dims, L)
+    shape = tuple(reversed(dims))
+    o = oracle_mod.Oracle(dims, np.float64)
+    o.set_coeff(L)
+    u = rng.standard_normal((n,) + shape) * L
+    b = o.divergence(u).ravel()
+    nb = np.abs(b).max()
+    if far:
+        p0 = 200.0 * rng.standard_normal(b.size)
+        tol = 1e-3
+    else:
+        p0 = np.zeros(b.size)
+        for _ in range(6):                       # six dense cycles towards the solution, mean NOT removed, then an offset
+            p0 = dense_vcycle(As, Rs, 0, p0, b)
+        p0 = p0 + 0.37
+        tol = 1e-4
+    r0 = np.abs(b - As[0] @ p0).max()
+    assert (r0 > 50 * nb) if far else (r0 < 1e-2 * nb)
+    k_nb, hist_nb = dense_solve_count(As, Rs, p0.copy(), b, tol, 64, nb)
+    k_r0, _ = dense_solve_count(As, Rs, p0.copy(), b, tol, 64, r0)
+    assert k_nb != k_r0 and 0 < k_nb < 64 and 0 < k_r0 < 64, (k_nb, k_r0)   # the case discriminates between the two readings
+    p, hist, nc, rc = o.solve(p0.reshape(shape), b.reshape(shape), tol, 64)
+    assert nc == k_nb and rc == 0, (nc, k_nb, k_r0)
+    assert hist.shape == hist_nb.shape
+    assert np.abs(hist / hist_nb - 1.0).max() <= 1e-9
+    assert hist[-1] <= tol * nb < hist[-2]
+    assert abs(p.mean()) <= 1e-13 * max(1.0, np.abs(p).max())
