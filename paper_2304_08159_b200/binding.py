@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libwl.so")
 WL_F32, WL_F64 = 0, 1
 WL_OK, WL_NOT_CONVERGED = 0, 1
 WL_EINVAL, WL_EDIMS, WL_ENOMEM, WL_ECUDA, WL_ESTATE = -1, -2, -3, -4, -5
-WL_OPT_FUSED, WL_OPT_GRAPH, WL_OPT_COARSE_CTA = 1, 2, 3
+WL_OPT_FUSED, WL_OPT_GRAPH, WL_OPT_COARSE_CTA, WL_OPT_SOLVE_KERNELS = 1, 2, 3, 4
 
 # every symbol include/wl.h declares: (restype, argtypes)
 _vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double

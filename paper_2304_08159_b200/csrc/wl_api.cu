@@ -55,7 +55,7 @@ struct wl_ctx {
     void* stage_L = nullptr;
     void* stage_p = nullptr;
     bool have_coeff = false;
-    int opt_fused = 1, opt_graph = 1, opt_coarse_cta = 1;
+    int opt_fused = 1, opt_graph = 1, opt_coarse_cta = 1, opt_solve_kernels = 0;
     int num_sms = 148;
     // cached CUDA graph of one V-cycle (H9), valid for one (p, b, variant, stream, options) combination
     cudaStream_t own_stream = nullptr;   // the legacy default stream cannot be captured: graphs then run here, fenced by events
@@ -227,15 +227,12 @@ struct Impl {
 
 
     // ---- fused level halves (wl_fused3d.cuh) ---------------------------------------------------------------------
-// Tile height / planes in flight of the fp32 3-D kernels (A/B switches).  Measured at 512^3: TY = 24 with 16 warps
-// (128 registers, 1 plane in flight) runs the DOWN kernel in 0.871 ms against 0.777 ms for TY = 16 with 12 warps.
-#ifndef WL_FTY32
-#define WL_FTY32 16
-#define WL_FPF_DOWN 3
-#define WL_FPF_UP 2
-#endif
-    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? WL_FTY32 : 14;   // 12 warps each
-    template <bool PROLONG> static constexpr int FPF = (PROLONG && WL_UP_LOADS_C) ? WL_FPF_UP : WL_FPF_DOWN;   // planes in flight: what fits 227 KB beside the ring
+    // Tile and planes in flight (what fits 227 KB beside the exchange planes).  fp32: 64x16 cells, omega/D recomputed in
+    // the kernel (5 planes per ring slot); fp64: 32x14 cells, omega/D read as a sixth plane (an IEEE fp64 division is ~20
+    // instructions).  12 warps each.  Measured alternatives: profiles/r2_fused_ncu.md.
+    static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? 16 : 14;
+    static constexpr bool USEC = sizeof(T) == 8;
+    template <bool PROLONG> static constexpr int FPF = (PROLONG && USEC) ? 2 : 3;
 
     // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
     // vectors; opt_fused == 1 keeps levels smaller than one tile on the generic kernels, 2 forces them (tests).
@@ -264,7 +261,7 @@ struct Impl {
         return encode_map(m, base, (int)sizeof(T), 2, d, b);
     }
 
-    template <bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS, bool RIN = false>
+    template <bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS, bool RIN = false, bool TICKET = false>
     static int launch_fused2(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out, void* bc) {
         using G = F2<T, F2TX, F2TY>;
         Level& f = c->lev[l];
@@ -281,10 +278,14 @@ struct Impl {
         prm.bc = P(bc);
         prm.scal = c->d_scal;
         prm.partials = c->d_partials;
+        prm.hist = c->d_hist;
+        prm.host_scal = c->h_scal;
+        prm.host_hist = c->h_hist;
+        prm.cells = f.g.M;
         prm.check_done = c->check_done;
         const int grid = prm.tiles_x * prm.tiles_y;
         c->fused_grid = grid;
-        k_fused2d<T, F2TX, F2TY, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN>
+        k_fused2d<T, F2TX, F2TY, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN, TICKET>
             <<<grid, G::NT, fused2d_smem_bytes<T, F2TX, F2TY>(), c->stream>>>(mx, mb, mL0, mL1, mxc, prm);
         KCHECK(c, "k_fused2d");
         return WL_OK;
@@ -298,7 +299,7 @@ struct Impl {
         return encode_map(m, base, (int)sizeof(T), 3, d, b);
     }
 
-    template <bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS, bool RIN = false>
+    template <bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS, bool RIN = false, bool TICKET = false>
     static int launch_fused(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out, void* bc) {
         if constexpr (ND == 3) {
             using G = F3<T, FTX, FTY>;
@@ -306,7 +307,8 @@ struct Impl {
             CUtensorMap mx, mb, mL0, mL1, mL2, mC, mxc;
             bool ok = map_cells(&mb, b, f.g, false);
             ok = ok && map_cells(&mL0, P(f.L), f.g, false) && map_cells(&mL1, P(f.L) + f.g.M, f.g, false) &&
-                 map_cells(&mL2, P(f.L) + 2 * f.g.M, f.g, false) && map_cells(&mC, P(f.C), f.g, false);
+                 map_cells(&mL2, P(f.L) + 2 * f.g.M, f.g, false);
+            if (USEC) ok = ok && map_cells(&mC, P(f.C), f.g, false); else mC = mb;
             if (ZERO_IN) mx = mb; else ok = ok && map_cells(&mx, x_in, f.g, false);
             if (PROLONG) ok = ok && map_cells(&mxc, xc, c->lev[l + 1].g, true); else mxc = mb;
             if (!ok) return fail(c, WL_ECUDA, "cuTensorMapEncodeTiled refused a level array (alignment?)");
@@ -331,9 +333,14 @@ struct Impl {
             prm.bc = P(bc);
             prm.scal = c->d_scal;
             prm.partials = c->d_partials;
+            prm.hist = c->d_hist;
+            prm.host_scal = c->h_scal;
+            prm.host_hist = c->h_hist;
+            prm.cells = f.g.M;
+            prm.negzero2 = 0x8000000080000000ULL;
             prm.check_done = c->check_done;
-            auto kern = k_fused3d<T, FTX, FTY, FPF<PROLONG>, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN>;
-            constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF<PROLONG>, PROLONG>();
+            auto kern = k_fused3d<T, FTX, FTY, FPF<PROLONG>, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN, USEC, TICKET>;
+            constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF<PROLONG>, PROLONG, USEC>();
             long long g = ntiles * best_nc;
             if (g > c->num_sms) g = c->num_sms;
             if (NORMS && g > kMaxPartials) g = kMaxPartials;
@@ -342,13 +349,15 @@ struct Impl {
             KCHECK(c, "k_fused3d");
             return WL_OK;
         } else {
-            return launch_fused2<PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN>(c, l, x_in, xc, b, x_out, bc);
+            return launch_fused2<PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN, TICKET>(c, l, x_in, xc, b, x_out, bc);
         }
     }
 
     // DOWN half of level l: x_out = J(J(x_in)) (x_in == nullptr: from zero), bc = R(b - A x_out).
     static int down(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out, void* bc) {
         if (!fused_ok(c, l)) return down_generic(c, l, x_in, b, x_out, bc);
+        if (c->opt_solve_kernels && l == 0 && x_in && c->d_hist)   // the instance wl_solve's graph launches (profiling / bench)
+            return launch_fused<false, false, true, true, true, false, true, true>(c, l, x_in, nullptr, b, x_out, bc);
         if (x_in) return launch_fused<false, false, false, true, true, false>(c, l, x_in, nullptr, b, x_out, bc);
         return launch_fused<false, true, false, true, true, false>(c, l, nullptr, nullptr, b, x_out, bc);
     }
@@ -356,6 +365,8 @@ struct Impl {
     // UP half of level l: x_out = J(J(x_in + P xc)).
     static int up(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out) {
         if (!fused_ok(c, l)) return up_generic(c, l, x_in, xc, b, x_out);
+        if (c->opt_solve_kernels && l == 0 && c->d_hist)
+            return launch_fused<true, false, false, false, false, true, false, true>(c, l, x_in, xc, b, x_out, nullptr);
         return launch_fused<true, false, false, false, false, false>(c, l, x_in, xc, b, x_out, nullptr);
     }
 
@@ -489,42 +500,36 @@ struct Impl {
         return WL_OK;
     }
 
-    // The solve cycle with the lagged stop test (k_cycle_check): DOWN0 measures the residual of its input for free, UP0
-    // needs no residual stage (2 stencil stages instead of 3) and only sums p.
+    // The solve cycle with the lagged stop test: DOWN0 measures the residual of its input for free and its
+    // last CTA records it and takes the stop decision; UP0 needs no residual stage (2 stencil stages instead of 3), only
+    // sums p, and its last CTA finishes the mean and bumps the cycle counter.  No single-thread kernels in the cycle.
     static int cycle_lagged(wl_ctx* c, void* p, const void* b) {
         int rc;
         Level& k1 = c->lev[1];
-        k_zero_slot<<<1, 32, 0, c->stream>>>(c->d_scal, 1);
-        KCHECK(c, "k_zero_slot");
-        if ((rc = launch_fused<false, false, true, true, true, false, true>(c, 0, p, nullptr, b, c->lev[0].x[1], k1.b))) return rc;
-        k_cycle_check<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, c->h_scal, c->h_hist);
-        KCHECK(c, "k_cycle_check");
+        if ((rc = launch_fused<false, false, true, true, true, false, true, true>(c, 0, p, nullptr, b, c->lev[0].x[1], k1.b))) return rc;
         if ((rc = vcycle(c, 1, nullptr, k1.b, k1.x[0], k1.x[1]))) return rc;
-        if ((rc = launch_fused<true, false, false, false, false, true, false>(c, 0, c->lev[0].x[1], k1.x[1], b, p, nullptr))) return rc;
-        k_finish_mean<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_partials, c->fused_grid, c->lev[0].g.M);
-        KCHECK(c, "k_finish_mean");
-        k_cycle_end_lagged<<<1, 32, 0, c->stream>>>(c->d_scal);
-        KCHECK(c, "k_cycle_end_lagged");
-        return WL_OK;
+        return launch_fused<true, false, false, false, false, true, false, true>(c, 0, c->lev[0].x[1], k1.x[1], b, p, nullptr);
     }
 
     // Set every opt-in shared-memory size once, outside any stream capture.
     static int init_kernels(wl_ctx* c) {
         if constexpr (ND == 3) {
-            constexpr size_t s0 = fused3d_smem_bytes<T, FTX, FTY, FPF<false>, false>(), s1 = fused3d_smem_bytes<T, FTX, FTY, FPF<true>, true>();
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, true, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s0));
-            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+            constexpr int s0 = (int)fused3d_smem_bytes<T, FTX, FTY, FPF<false>, false, USEC>(), s1 = (int)fused3d_smem_bytes<T, FTX, FTY, FPF<true>, true, USEC>();
+            constexpr auto A = cudaFuncAttributeMaxDynamicSharedMemorySize;
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, false, true, true, false, false, USEC, false>, A, s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, true, false, true, true, false, false, USEC, false>, A, s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, false, false, false, false, USEC, false>, A, s1));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, true, true, true, false, true, USEC, true>, A, s0));
+            CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<true>, true, false, false, false, false, true, false, USEC, true>, A, s1));
         }
         if constexpr (ND == 2) {
             constexpr int s2 = (int)fused2d_smem_bytes<T, F2TX, F2TY>();
-            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
-            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, true, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
-            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
-            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, true, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
-            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s2));
+            constexpr auto A = cudaFuncAttributeMaxDynamicSharedMemorySize;
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, false, true, true, false, false, false>, A, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, true, false, true, true, false, false, false>, A, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, false, false, false>, A, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, false, false, true, true, true, false, true, true>, A, s2));
+            CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, true, false, true>, A, s2));
         }
         CU(c, cudaFuncSetAttribute(k_coarse_tail<T, ND>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTailSmemBudget));
         return WL_OK;
@@ -878,6 +883,7 @@ int wl_set_option(wl_ctx* c, int key, int value) {
         case WL_OPT_FUSED: c->opt_fused = (value < 0 || value > 2) ? 1 : value; return WL_OK;
         case WL_OPT_GRAPH: c->opt_graph = value ? 1 : 0; return WL_OK;
         case WL_OPT_COARSE_CTA: c->opt_coarse_cta = value ? 1 : 0; return WL_OK;
+        case WL_OPT_SOLVE_KERNELS: c->opt_solve_kernels = value ? 1 : 0; return WL_OK;
         default: return fail(c, WL_EINVAL, "wl_set_option: unknown key");
     }
 }
@@ -982,6 +988,7 @@ int wl_down(wl_ctx* c, int level, const void* x_in, const void* b, void* x_out, 
     if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_down: bad level") : WL_EINVAL;
     if (!b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_down: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_down: coefficients not set");
+    if (c->opt_solve_kernels) { int rc = ensure_hist(c, 63); if (rc) return rc; }
     return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
 }
 
@@ -989,6 +996,7 @@ int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b,
     if (level_check(c, level, true)) return c ? fail(c, WL_EINVAL, "wl_up: bad level") : WL_EINVAL;
     if (!x_in || !b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_up: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_up: coefficients not set");
+    if (c->opt_solve_kernels) { int rc = ensure_hist(c, 63); if (rc) return rc; }
     return DISPATCH(c, up)(c, level, x_in, xc ? xc : c->lev[level + 1].x[1], b, x_out);
 }
 

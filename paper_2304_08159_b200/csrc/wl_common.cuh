@@ -27,7 +27,7 @@ struct Scalars {
     int cycle;                          // cycles completed in the running solve
     int done;                           // 1 once hist[cycle] <= tol * nb
     int maxcycles;
-    int pad;
+    unsigned int ticket;                // CTAs of the running level-0 launch that have finished (last one does the bookkeeping)
 };
 
 template <typename T> struct Omega;
@@ -75,6 +75,41 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
 
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* slot, double v) {
     atomicMax(slot, (unsigned long long)__double_as_longlong(v));
+}
+
+// ---- solve bookkeeping of the lagged stop test, run by the LAST CTA of the level-0 launches -------------
+// After the level-0 DOWN launch g of a solve: slot 1 holds ||b - A p_k||inf of its INPUT p_k (k = g-1 cycles done; k = 0: the
+// caller's initial guess).  Record it as hist[k], take the stop decision, mirror to the pinned host copy, clear the slot for
+// the next launch.  When it stops, every later kernel of this and of the next (already enqueued) launch returns at once
+// (check_done) and p still holds p_k: the DOWN kernel writes scratch only.  One thread.
+__device__ __forceinline__ void solve_check_lagged(Scalars* scal, double* __restrict__ hist, Scalars* host_mirror,
+                                                   double* host_hist) {
+    const int k = scal->cycle;
+    const double r = __longlong_as_double((long long)scal->absmax_bits[1]);
+    scal->absmax_bits[1] = 0ULL;
+    if (k > scal->maxcycles) return;   // cannot happen inside a solve (done is set at k = maxcycles); keeps stand-alone launches in bounds
+    hist[k] = r;
+    if (!(r > scal->tol * scal->nb) || k >= scal->maxcycles) scal->done = 1;
+    host_hist[k] = r;
+    host_mirror->nb = scal->nb;
+    __threadfence_system();
+    *((volatile int*)&host_mirror->cycle) = k + 1;   // number of history entries the host may read
+}
+// After the level-0 UP launch: mean_p = (sum of the per-CTA partials in a FIXED order) / M — lane l adds partials l, l+32,
+// ... in sequence, a shuffle tree combines the 32 lane sums: the same order on every run (bit-reproducible) — then the
+// cycle counter and the shift the next DOWN launch subtracts on load.  One warp (all 32 lanes must call).
+__device__ __forceinline__ void solve_finish_mean_lagged(Scalars* scal, const double* partials, int nparts, long long M) {
+    const int lane = threadIdx.x & 31;
+    double s = 0.0;
+    for (int i = lane; i < nparts; i += 32) s += ((const volatile double*)partials)[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if (lane == 0) {
+        scal->sum_p = s;
+        scal->mean_p = s / (double)M;
+        scal->cycle += 1;
+        scal->shift = scal->mean_p;
+    }
 }
 
 }  // namespace wl

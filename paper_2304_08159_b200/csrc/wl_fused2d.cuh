@@ -8,7 +8,7 @@
 // shrinking rings with one __syncthreads between them, x1 and x2 live in shared memory only; a thread owns VEC
 // consecutive cells (16 bytes) of a row and walks rows with stride RP.  2-D levels are small (BASELINE config 1:
 // 4 MiB per array, L2-resident), so the kernel is latency-, not bandwidth-bound: one tile per CTA, several CTAs per SM.
-// Expression order = the oracle's (upper face, lower face; axis 0, then 1; D summed per axis).
+// Expression order = the oracle's (upper face, lower face; axis 0, then 1; D summed per axis; IEEE division).
 #pragma once
 #include "wl_common.cuh"
 #include "wl_fused3d.cuh"
@@ -44,6 +44,10 @@ struct Fused2Params {
     T* bc;
     Scalars* scal;
     double* partials;
+    double* hist;            // [TICKET] solve bookkeeping, as in Fused3Params
+    Scalars* host_scal;
+    double* host_hist;
+    long long cells;
     int check_done;
 };
 
@@ -75,7 +79,7 @@ __device__ __forceinline__ void apply_A2(const T* __restrict__ l0, const T* __re
     }
 }
 
-template <typename T, int TX, int TY, bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS, bool RIN = false>
+template <typename T, int TX, int TY, bool PROLONG, bool ZERO_IN, bool SHIFT, bool STAGE3, bool RESTRICT, bool NORMS, bool RIN, bool TICKET>
 __global__ void __launch_bounds__(F2<T, TX, TY>::NT)
 k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUtensorMap tm_b,
           const __grid_constant__ CUtensorMap tm_L0, const __grid_constant__ CUtensorMap tm_L1,
@@ -150,7 +154,7 @@ k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUte
                 for (int v = 0; v < VEC; ++v) {
                     const T Lxp = (v + 1 < VEC) ? L0[(v + 1) % VEC] : L0n;
                     const T Dv = (L0[v] + Lxp) + (L1[v] + L1p[v]);
-                    const T c = (Dv > (T)0) ? omega * recip_fast(Dv) : (T)0;
+                    const T c = (Dv > (T)0) ? omega * ((T)1 / Dv) : (T)0;
                     x1[v] = c * ((T)0 - bb[v]);
                 }
             } else {
@@ -159,7 +163,7 @@ k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUte
                 const bool inside = tx >= G::TX0 && tx < G::TX1 && ty >= G::HY && ty < WY - G::HY && gx < P.N0 && gy < P.N1;
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) {
-                    const T c = (D[v] > (T)0) ? omega * recip_fast(D[v]) : (T)0;
+                    const T c = (D[v] > (T)0) ? omega * ((T)1 / D[v]) : (T)0;
                     const T d = Ax[v] - bb[v];
                     if constexpr (RIN) {
                         if (inside) rmax = fmax(rmax, fabs(d));
@@ -180,7 +184,7 @@ k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUte
             apply_A2<T, VEC, WX>(sl0, sl1, sx1, me, xc, Ax, D);
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
-                const T c = (D[v] > (T)0) ? omega * recip_fast(D[v]) : (T)0;
+                const T c = (D[v] > (T)0) ? omega * ((T)1 / D[v]) : (T)0;
                 x2[v] = xc[v] + c * (Ax[v] - bb[v]);
             }
             st_vec<T, VEC>(sx2 + me, x2);
@@ -243,6 +247,24 @@ k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUte
         if constexpr (NORMS) {
             const double s = block_sum(psum, red);
             if (t == 0) P.partials[blockIdx.x] = s;
+        }
+        if constexpr (TICKET) {   // the last CTA to finish does the cycle's bookkeeping (wl_fused3d.cuh)
+            __shared__ int s_last;
+            if (t == 0) {
+                __threadfence();
+                const unsigned int ticket = atomicAdd(&P.scal->ticket, 1u);
+                s_last = (ticket == gridDim.x - 1) ? 1 : 0;
+            }
+            __syncthreads();
+            if (s_last && t < 32) {
+                __threadfence();
+                if constexpr (RIN) {
+                    if (t == 0) solve_check_lagged(P.scal, P.hist, P.host_scal, P.host_hist);
+                } else {
+                    solve_finish_mean_lagged(P.scal, P.partials, (int)gridDim.x, P.cells);
+                }
+                if (t == 0) P.scal->ticket = 0u;
+            }
         }
     }
 }

@@ -329,28 +329,13 @@ __global__ void k_cycle_end(Scalars* scal, double* __restrict__ hist, int deferr
     }
 }
 
-// Lagged stop test (wl_solve when every level is fused or in the tail): launch g of the cycle graph begins with the
-// level-0 DOWN kernel, which read ||b - A p_k||inf of its INPUT p_k = result of cycle k = g-1 (after the mean shift,
-// exactly the oracle's iterate; k = 0: the caller's initial guess) off its first sweep.  Record it as hist[k], take the
-// stop decision, mirror to the host.  When it stops, the rest of this launch returns at once (check_done) and
-// p still holds p_k: the DOWN kernel writes scratch only.
-__global__ void k_cycle_check(Scalars* scal, double* __restrict__ hist, Scalars* host_mirror, double* host_hist) {
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
-        if (scal->done) return;
-        const int k = scal->cycle;   // k = 0: the initial residual, read off the first launch's DOWN kernel
-        const double r = __longlong_as_double((long long)scal->absmax_bits[1]);
-        hist[k] = r;
-        if (!(r > scal->tol * scal->nb) || k >= scal->maxcycles) scal->done = 1;
-        host_hist[k] = r;
-        host_mirror->nb = scal->nb;
-        __threadfence_system();
-        *((volatile int*)&host_mirror->cycle) = k + 1;   // number of history entries the host may read
-    }
-}
-// Lagged solve: nb from slot 0 (||b||inf), nothing else is known yet.
+// Lagged solve (the stop test rides on the level-0 launches: solve_check_lagged / solve_finish_mean_lagged in wl_common.cuh):
+// nb from slot 0 (||b||inf), nothing else is known yet; slot 1 and the CTA ticket start at 0.
 __global__ void k_solve_begin_lagged(Scalars* scal, double tol, int maxcycles) {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         scal->nb = __longlong_as_double((long long)scal->absmax_bits[0]);
+        scal->absmax_bits[1] = 0ULL;
+        scal->ticket = 0u;
         scal->tol = tol;
         scal->maxcycles = maxcycles;
         scal->cycle = 0;
@@ -358,12 +343,4 @@ __global__ void k_solve_begin_lagged(Scalars* scal, double tol, int maxcycles) {
         scal->done = 0;
     }
 }
-__global__ void k_cycle_end_lagged(Scalars* scal) {
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
-        if (scal->done) return;
-        scal->cycle += 1;
-        scal->shift = scal->mean_p;
-    }
-}
-
 }  // namespace wl
