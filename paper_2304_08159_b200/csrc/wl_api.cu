@@ -232,7 +232,7 @@ struct Impl {
     // instructions).  12 warps each.  Measured alternatives: profiles/r2_fused_ncu.md.
     static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? 16 : 14;
     static constexpr bool USEC = sizeof(T) == 8;
-    template <bool PROLONG> static constexpr int FPF = (PROLONG && USEC) ? 2 : 3;
+    template <bool PROLONG> static constexpr int FPF = (PROLONG && USEC) ? 2 : 3;   // fp32 DOWN with 4 planes in flight: no gain
 
     // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
     // vectors; opt_fused == 1 keeps levels smaller than one tile on the generic kernels, 2 forces them (tests).
