@@ -12,14 +12,17 @@ The JSON line (rank 0):
              inputs resident in HBM when the timed region starts (CUDA events on the ctx stream, summed over K steps);
   e2e        the same metric through ``wl_project_host`` with pinned HOST buffers: H2D of u, L, p and D2H of u, p inside
              the timed region;
-  roofline   the dominant kernel (the fused level-0 DOWN kernel: 2 pre-sweeps + residual + restriction) timed alone with
-             CUDA events through ``wl_down``; achieved = algorithmic bytes (read p, b, n·L, write p, write
-             b_c = (n+3+1/2^n)·s per cell) / duration, against MEASURED_PEAKS.json ``hbm_gbs``;
+  roofline   the dominant kernel — the fused level-0 DOWN kernel of the solve (mean shift on load, 2 pre-sweeps, residual of
+             the input iterate, residual + restriction, bookkeeping ticket: the very template instance wl_solve's graph
+             launches, selected through WL_OPT_SOLVE_KERNELS) — timed alone with CUDA events through ``wl_down``; achieved =
+             algorithmic bytes (read p, b, n·L, write p, write b_c = (n+3+1/2^n)·s per cell) / duration,
+             against MEASURED_PEAKS.json ``hbm_gbs`` (``frac``) and against the nominal 8 TB/s BASELINE.json names;
   cpu_baseline  the oracle as it stands on the box's host cores (1 thread), on a bounded sample (one V-cycle of the same
              workload);
   extra keys: ms per projection, ms per V-cycle (wl_solve with tol = 0 over --kernel-reps cycles: one graph launch per
-             cycle, stop test on the device), effective GB/s per V-cycle (56 B/cell model); roofline.traffic = DRAM bytes of
-             one DOWN launch from the last ncu capture under profiles/ (a recorded constant, ncu never runs here).
+             cycle, stop test on the device), effective GB/s per V-cycle (56 B/cell model) as a fraction of the measured and
+             of the nominal peak; roofline.traffic = DRAM bytes of one DOWN launch from profiles/traffic.json (written from
+             the last ``ncu --set full`` capture together with a hash of csrc/; null when the kernels have changed since).
 
 N > 1 (torchrun): "replicas only" — every rank projects its own copy of the grid, no collective on the data path
 (BASELINE.json north_star: one GPU, no sharding); value = units all ranks processed / max-over-ranks time.
@@ -70,8 +73,33 @@ def whole_job_value(world: int, cells: int, cycles: int, seconds_per_step: float
     return world * cells * cycles / seconds_per_step if (cycles > 0 and seconds_per_step > 0) else 0.0
 
 
-# DRAM traffic of one level-0 DOWN launch at 512^3 fp32 from the last `ncu --set full` capture (profiles/): bytes.
-NCU_TRAFFIC_DOWN_512 = 3.959e9   # profiles/r1_fused_ncu.md (capture r1_fused_v16_c4): 3.367 GB read + 0.591 GB written
+NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star: "the B200's ~8 TB/s HBM peak"
+
+
+def csrc_hash() -> str:
+    """sha256 over the CUDA sources and the C header: identifies the kernels a recorded ncu number belongs to."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    files = sorted(glob.glob(os.path.join(ROOT, "paper_2304_08159_b200", "csrc", "*.cu*"))) + [os.path.join(ROOT, "include", "wl.h")]
+    for f in files:
+        with open(f, "rb") as fh:
+            h.update(os.path.basename(f).encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def recorded_traffic(workload: str, kernel_key: str):
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of one launch of `kernel_key` on `workload` from
+    profiles/traffic.json, or None if there is no record for the kernels as they are now (ncu never runs inside bench.py)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            rec = json.load(f)
+        if rec.get("csrc_hash") != csrc_hash():
+            return None
+        e = rec["kernels"][workload][kernel_key]
+        return float(e["dram_bytes_read"]) + float(e["dram_bytes_write"])
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -285,6 +313,7 @@ def main():
 
         kern = {}
         if pr.num_levels > 1:
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 1)   # time the instances the solve's graph launches
             xo = pr.empty_cells()
             for name, fn in (("down", lambda: wl.wl_down(pr.ctx, 0, p, bd, xo)),
                              ("up", lambda: wl.wl_up(pr.ctx, 0, xo, None, bd, p))):
@@ -314,12 +343,19 @@ def main():
     if kern:
         bytes_down = _algorithmic_bytes_down(n, esz) * M
         ach = bytes_down / (kern["down"]["ms"] * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "level-0 DOWN (2 pre-sweeps + residual + restriction), via wl_down",
+        fused3 = (n == 3 and args.fused != 0)
+        roof = {"bound": "hbm",
+                "kernel": ("level-0 DOWN of the solve: k_fused3d<SHIFT, STAGE3, RESTRICT, RIN, TICKET> (mean shift on load, 2 pre-sweeps, "
+                           "input-residual norm, residual + restriction, bookkeeping), via wl_down with WL_OPT_SOLVE_KERNELS") if fused3
+                          else "level-0 DOWN half (2 pre-sweeps + residual + restriction), via wl_down",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": NCU_TRAFFIC_DOWN_512 if (args.config == 4 and args.scale == 1 and not args.donut and dt == np.float32) else None,
+                "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS,
+                "traffic": recorded_traffic(cfg["name"], "down"),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_down,
                 "launches_per_call": kern["down"]["launches_per_call"], "ms": kern["down"]["ms"],
                 "up_kernel": {"ms": kern["up"]["ms"], "achieved": bytes_down / (kern["up"]["ms"] * 1e-3) / 1e9,
+                              "frac": bytes_down / (kern["up"]["ms"] * 1e-3) / 1e9 / peak,
+                              "traffic": recorded_traffic(cfg["name"], "up"),
                               "launches_per_call": kern["up"]["launches_per_call"]}}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -330,8 +366,9 @@ def main():
                    "l2": "inputs larger than L2 (no flush needed)" if (n + 3) * M * esz > 200e6 else "working set fits L2",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "ms_per_projection": sec_per_step * 1e3,
-        "vcycle": {"ms": vcycle_ms, "cells_per_s": M / (vcycle_ms * 1e-3),
-                   "effective_GBps_56B_model": (2 * (n + 3) + 2.0 / 2 ** n) * esz * (2 ** n / (2 ** n - 1.0)) * M / (vcycle_ms * 1e-3) / 1e9},
+        "vcycle": (lambda eff: {"ms": vcycle_ms, "cells_per_s": M / (vcycle_ms * 1e-3), "effective_GBps_56B_model": eff,
+                                "frac_of_measured": eff / peak, "frac_of_nominal_8TBs": eff / NOMINAL_HBM_GBS})(
+            (2 * (n + 3) + 2.0 / 2 ** n) * esz * (2 ** n / (2 ** n - 1.0)) * M / (vcycle_ms * 1e-3) / 1e9),
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": roof,

@@ -50,6 +50,7 @@ def lib():
         L.orc_vcycle.restype, L.orc_vcycle.argtypes = f64, [vp, vp, vp]
         L.orc_solve.restype, L.orc_solve.argtypes = i32, [vp, vp, vp, f64, i32, f64p, i32p]
         L.orc_project.restype, L.orc_project.argtypes = i32, [vp, vp, vp, vp, f64, i32, f64p, i32p]
+        L.orc_solve_pcg.restype, L.orc_solve_pcg.argtypes = i32, [vp, vp, vp, f64, i32, f64p, i32p]
         L.orc_divergence.restype, L.orc_divergence.argtypes = None, [vp, vp, vp]
         L.orc_gradient_correct.restype, L.orc_gradient_correct.argtypes = None, [vp, vp, vp]
         L.orc_remove_mean.restype, L.orc_remove_mean.argtypes = None, [vp, vp]
@@ -158,6 +159,16 @@ class Oracle:
         rc = lib().orc_solve(self._h, _ptr(p), _ptr(b), float(tol), int(maxcycles),
                              hist.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), ctypes.byref(nc))
         return p, hist[: nc.value + 1].copy(), nc.value, rc
+
+    def solve_pcg(self, p, b, tol: float, maxit: int):
+        """V-cycle-preconditioned conjugate gradients (NEXT-1).  Returns (p, hist[0..nit], nit, rc)."""
+        p = self._c(p, self.cell_shape(0)).copy()
+        b = self._c(b, self.cell_shape(0))
+        hist = np.zeros(maxit + 1, dtype=np.float64)
+        nit = ctypes.c_int(0)
+        rc = lib().orc_solve_pcg(self._h, _ptr(p), _ptr(b), float(tol), int(maxit),
+                                 hist.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), ctypes.byref(nit))
+        return p, hist[: nit.value + 1].copy(), nit.value, rc
 
     def project(self, u, L, p, tol: float, maxcycles: int):
         """Returns (u_new, p, hist, ncycles, rc).  ``L=None`` keeps the current coefficients."""

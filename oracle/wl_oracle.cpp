@@ -25,6 +25,15 @@
 //   divergence, gradient_correct, project
 //                  pinned: div(u_out) == b - A p to rounding; max|div u_out| <= tol·max|b| when
 //                  converged; -G^T / G incidence forms.
+//   solve_pcg      ("Conjugate-Gradient ... within the GMG")
+//                  pinned: textbook preconditioned CG written with dense NumPy matrices (the
+//                  preconditioner = the dense-matrix V-cycle of tests/test_oracle_cycle.py applied
+//                  to unit vectors), iterate by iterate; M^-1-orthogonality of the residuals and
+//                  A-conjugacy of the directions; termination on the dense pseudo-inverse solution
+//                  in <= rank(A) steps on tiny grids (tests/test_oracle_pcg.py).  The reading
+//                  (V-cycle as preconditioner, where the mean is removed, fp64 dot products) is
+//                  DESIGN.md section 3 reading 13: the paper gives no detail -> "parity unpinned" by any
+//                  value of the paper.
 //
 // Notation: n = ndim in {2,3}; N = (N_0..N_{n-1}), axis 0 unit-stride; cell I has
 // linear index I_0 + N_0 (I_1 + N_1 I_2); face (I,i) is the LOWER face of cell I in direction i
@@ -387,6 +396,62 @@ int ctx_solve(Ctx<T>* c, T* p, const T* b, double tol, int maxcycles, double* hi
     return (hist[k] > tol * nb) ? 1 : 0;
 }
 
+// SOLVE_PCG — conjugate gradients on A p = b with ONE V-cycle (from a zero guess) as the
+// preconditioner ("we now use Conjugate-Gradient smoothing within the GMG levels";
+// reading 13 of DESIGN.md section 3: CG is wrapped around the multigrid cycle, the cycle itself —
+// Jacobi sweeps, transfers, 64 coarse sweeps — stays the one of BJ).  A is negative semi-definite,
+// the formulas are the textbook ones written with A itself (the two sign changes cancel):
+//   r = b - A x;  hist[0] = ||r||inf
+//   repeat while k < K and hist[k] > tol·||b||inf:
+//     z = VCYCLE(0) applied to A z = r from z = 0;  mz = (T) mean(z)         (sum in fp64)
+//     rho' = sum r_i z_i  (fp64, z before the shift);  beta = (T)(rho'/rho)  (first step: p = z - mz)
+//     p = (z - mz) + beta p;  q = A p;  sigma = sum p_i q_i (fp64);  alpha = (T)(rho'/sigma)
+//     x += alpha p;  r -= alpha q;  k++;  hist[k] = ||r||inf                  (recurrence residual)
+//   x -= mean(x)
+// Stops early (as converged) if rho' or sigma is exactly 0 (r = 0: nothing left to correct).
+template <class T>
+int ctx_solve_pcg(Ctx<T>* c, T* x, const T* b, double tol, int maxit, double* hist, int* nit) {
+    Level<T>& f = c->lev[0];
+    const int64_t M = f.g.M;
+    std::vector<T> r((size_t)M), z((size_t)M), p((size_t)M, (T)0), q((size_t)M);
+    const double nb = max_abs(b, M);
+    residual(f.g, f.L.data(), x, b, r.data());
+    hist[0] = max_abs(r.data(), M);
+    double rho = 0;
+    int k = 0;
+    while (k < maxit && hist[k] > tol * nb) {
+        std::fill(z.begin(), z.end(), (T)0);
+        vcycle(c, 0, z.data(), r.data());                                 // z ~ A^-1 r
+        double sz = 0, rho_new = 0;
+        for (int64_t I = 0; I < M; ++I) { sz += (double)z[I]; rho_new += (double)r[I] * (double)z[I]; }
+        const T mz = (T)(sz / (double)M);
+        if (rho_new == 0.0) break;
+        const T beta = (k == 0) ? (T)0 : (T)(rho_new / rho);
+        for (int64_t I = 0; I < M; ++I) {
+            const T zs = z[I] - mz;
+            const T bp = beta * p[I];
+            p[I] = zs + bp;
+        }
+        rho = rho_new;
+        apply_A(f.g, f.L.data(), p.data(), q.data());
+        double sigma = 0;
+        for (int64_t I = 0; I < M; ++I) sigma += (double)p[I] * (double)q[I];
+        if (sigma == 0.0) break;
+        const T alpha = (T)(rho / sigma);
+        for (int64_t I = 0; I < M; ++I) {
+            const T ap = alpha * p[I];
+            x[I] = x[I] + ap;
+            const T aq = alpha * q[I];
+            r[I] = r[I] - aq;
+        }
+        ++k;
+        hist[k] = max_abs(r.data(), M);
+    }
+    remove_mean(x, M);
+    *nit = k;
+    return (hist[k] > tol * nb) ? 1 : 0;
+}
+
 // PROJECT (PAPER.md:29-33 + BJ "wl_project(u, L, p), which computes the divergence, solves, and
 // corrects u").
 template <class T>
@@ -511,6 +576,14 @@ int orc_solve(void* hv, void* p, const void* b, double tol, int maxcycles, doubl
     int rc = 0;
     DISPATCH(h, rc = ctx_solve(c, (T*)p, (const T*)b, tol, maxcycles, hist, ncycles),
                 rc = ctx_solve(c, (T*)p, (const T*)b, tol, maxcycles, hist, ncycles));
+    return rc;
+}
+
+int orc_solve_pcg(void* hv, void* p, const void* b, double tol, int maxit, double* hist, int* nit) {
+    Handle* h = (Handle*)hv;
+    int rc = 0;
+    DISPATCH(h, rc = ctx_solve_pcg(c, (T*)p, (const T*)b, tol, maxit, hist, nit),
+                rc = ctx_solve_pcg(c, (T*)p, (const T*)b, tol, maxit, hist, nit));
     return rc;
 }
 
