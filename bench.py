@@ -205,6 +205,7 @@ def main():
     ap.add_argument("--dtype", default=None, choices=[None, "float32", "float64"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-pcg", action="store_true", help="skip the conjugate-gradient leg (reported beside the V-cycle solver)")
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--graph", type=int, default=1)
     ap.add_argument("--kernel-reps", type=int, default=20)
@@ -295,6 +296,19 @@ def main():
                     e2e_ms.append(e0.elapsed_time(e1))
             e2e_total = float(np.sum(e2e_ms))
 
+        # NEXT-1 beside the specified solver: the same projection with V-cycle-preconditioned conjugate gradients
+        pcg = None
+        if not args.no_pcg:
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVER, 1)
+            pms = []
+            for it in range(1 + max(2, args.steps)):
+                tms, hp, ncp, rcp = one_step()
+                if it >= 1:
+                    pms.append(tms)
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVER, 0)
+            pcg = {"solver": "wl_solve_pcg (one V-cycle per CG iteration)", "iterations": int(ncp), "converged": bool(rcp == 0),
+                   "ms_per_projection": float(np.mean(pms)), "final_rel_residual": float(hp[-1] / hp[0]) if hp[0] > 0 else 0.0}
+
         # V-cycles alone: wl_solve with tol = 0 runs exactly `reps` cycles (one graph launch + one 8-byte readback each,
         # mean shift deferred into the next cycle); the dominant kernels alone follow
         bd = pr.empty_cells()
@@ -369,6 +383,7 @@ def main():
         "vcycle": (lambda eff: {"ms": vcycle_ms, "cells_per_s": M / (vcycle_ms * 1e-3), "effective_GBps_56B_model": eff,
                                 "frac_of_measured": eff / peak, "frac_of_nominal_8TBs": eff / NOMINAL_HBM_GBS})(
             (2 * (n + 3) + 2.0 / 2 ** n) * esz * (2 ** n / (2 ** n - 1.0)) * M / (vcycle_ms * 1e-3) / 1e9),
+        "pcg": pcg,
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": roof,

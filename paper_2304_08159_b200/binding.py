@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libwl.so")
 WL_F32, WL_F64 = 0, 1
 WL_OK, WL_NOT_CONVERGED = 0, 1
 WL_EINVAL, WL_EDIMS, WL_ENOMEM, WL_ECUDA, WL_ESTATE = -1, -2, -3, -4, -5
-WL_OPT_FUSED, WL_OPT_GRAPH, WL_OPT_COARSE_CTA, WL_OPT_SOLVE_KERNELS = 1, 2, 3, 4
+WL_OPT_FUSED, WL_OPT_GRAPH, WL_OPT_COARSE_CTA, WL_OPT_SOLVE_KERNELS, WL_OPT_SOLVER = 1, 2, 3, 4, 5
 
 # every symbol include/wl.h declares: (restype, argtypes)
 _vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double
@@ -31,6 +31,7 @@ SIGNATURES = {
     "wl_set_coeff": (_i32, [_vp, _vp]),
     "wl_vcycle": (_i32, [_vp, _vp, _vp, _f64p]),
     "wl_solve": (_i32, [_vp, _vp, _vp, _f64, _i32, _f64p, _i32p]),
+    "wl_solve_pcg": (_i32, [_vp, _vp, _vp, _f64, _i32, _f64p, _i32p]),
     "wl_project": (_i32, [_vp, _vp, _vp, _vp, _f64, _i32, _f64p, _i32p]),
     "wl_project_host": (_i32, [_vp, _vp, _vp, _vp, _f64, _i32, _f64p, _i32p]),
     "wl_divergence": (_i32, [_vp, _vp, _vp]),
@@ -144,6 +145,15 @@ def wl_solve(ctx, p, b, tol: float, maxcycles: int):
                          hist.ctypes.data_as(_f64p), ctypes.byref(nc))
     _check(ctx, rc, "wl_solve")
     return hist[: nc.value + 1].copy(), nc.value, rc
+
+
+def wl_solve_pcg(ctx, p, b, tol: float, maxit: int):
+    """V-cycle-preconditioned conjugate gradients.  Returns (hist[0..nit] as float64 ndarray, nit, rc)."""
+    hist = np.zeros(maxit + 1, dtype=np.float64)
+    nit = ctypes.c_int(0)
+    rc = load().wl_solve_pcg(ctx, _dptr(p), _dptr(b), float(tol), int(maxit), hist.ctypes.data_as(_f64p), ctypes.byref(nit))
+    _check(ctx, rc, "wl_solve_pcg")
+    return hist[: nit.value + 1].copy(), nit.value, rc
 
 
 def wl_project(ctx, u, L, p, tol: float, maxcycles: int):

@@ -16,6 +16,7 @@
 #include "wl_fused2d.cuh"
 #include "wl_tail.cuh"
 #include "wl_rows.cuh"
+#include "wl_pcg.cuh"
 
 using namespace wl;
 
@@ -51,6 +52,8 @@ struct wl_ctx {
     double* h_hist = nullptr;    // pinned
     int hist_cap = 0;
     void* b0 = nullptr;          // ctx-owned right-hand side for wl_project
+    void* cg_v[4] = {nullptr, nullptr, nullptr, nullptr};   // r, z, p, q of the conjugate-gradient solve (allocated on first use)
+    int opt_solver = 0;          // WL_OPT_SOLVER: 0 = V-cycles (BJ), 1 = V-cycle-preconditioned CG (NEXT-1)
     void* stage_u = nullptr;     // device staging for wl_project_host
     void* stage_L = nullptr;
     void* stage_p = nullptr;
@@ -511,6 +514,33 @@ struct Impl {
         return launch_fused<true, false, false, false, false, true, false, true>(c, 0, c->lev[0].x[1], k1.x[1], b, p, nullptr);
     }
 
+    // ---- V-cycle-preconditioned conjugate gradients (wl_pcg.cuh) ------------------------------------
+    static int pcg_residual(wl_ctx* c, const void* x, const void* b) {
+        Level& f = c->lev[0];
+        k_pcg_residual<T, ND><<<nparts_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, P(f.L), P(x), P(b), P(c->cg_v[0]), c->d_scal, c->d_hist,
+                                                                           c->h_scal, c->h_hist);
+        KCHECK(c, "k_pcg_residual");
+        return WL_OK;
+    }
+    // one iteration: z = V(r); rho', beta; p; q = A p, alpha; x, r, hist
+    static int pcg_iteration(wl_ctx* c, void* x) {
+        Level& f = c->lev[0];
+        const long long M = f.g.M;
+        T* r = P(c->cg_v[0]); T* z = P(c->cg_v[1]); T* p = P(c->cg_v[2]); T* q = P(c->cg_v[3]);
+        int rc;
+        if ((rc = vcycle(c, 0, nullptr, r, f.x[1], z))) return rc;
+        const int np = nparts_for(c, M) < kMaxPartials / 2 ? nparts_for(c, M) : kMaxPartials / 2;
+        k_pcg_dot_rz<T><<<np, kBlock, 0, c->stream>>>(M, r, z, c->d_scal, c->d_partials);
+        KCHECK(c, "k_pcg_dot_rz");
+        k_pcg_update_p<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, z, p, c->d_scal);
+        KCHECK(c, "k_pcg_update_p");
+        k_pcg_Ap<T, ND><<<np, kBlock, 0, c->stream>>>(f.g, P(f.L), p, q, c->d_scal, c->d_partials);
+        KCHECK(c, "k_pcg_Ap");
+        k_pcg_update_xr<T><<<np, kBlock, 0, c->stream>>>(M, P(x), r, p, q, c->d_scal, c->d_hist, c->h_scal, c->h_hist);
+        KCHECK(c, "k_pcg_update_xr");
+        return WL_OK;
+    }
+
     // Set every opt-in shared-memory size once, outside any stream capture.
     static int init_kernels(wl_ctx* c) {
         if constexpr (ND == 3) {
@@ -603,16 +633,16 @@ void drop_graph(wl_ctx* c) {
 }
 
 // One V-cycle (+ k_cycle_end bookkeeping when `in_solve`) on the ctx stream: a cached CUDA graph when WL_OPT_GRAPH is on.
-// variant: bit 0 = in_solve, bit 1 = lagged.
-int run_cycle(wl_ctx* c, void* p, const void* b, bool in_solve, bool lagged) {
+// variant: bit 0 = in_solve, bit 1 = lagged, 4 = one conjugate-gradient iteration (p = the iterate x, b unused).
+int run_cycle(wl_ctx* c, void* p, const void* b, bool in_solve, bool lagged, bool pcg = false) {
     int rc;
-    const int variant = (in_solve ? 1 : 0) | (lagged ? 2 : 0);
+    const int variant = pcg ? 4 : ((in_solve ? 1 : 0) | (lagged ? 2 : 0));
     auto enqueue = [&]() -> int {
         c->check_done = in_solve ? 1 : 0;
-        int r = lagged ? DISPATCH(c, cycle_lagged)(c, p, b) : DISPATCH(c, cycle)(c, p, b);
+        int r = pcg ? DISPATCH(c, pcg_iteration)(c, p) : (lagged ? DISPATCH(c, cycle_lagged)(c, p, b) : DISPATCH(c, cycle)(c, p, b));
         c->check_done = 0;
         if (r) return r;
-        if (in_solve && !lagged) {
+        if (in_solve && !lagged && !pcg) {
             k_cycle_end<<<1, 32, 0, c->stream>>>(c->d_scal, c->d_hist, 0, c->h_scal, c->h_hist);
             KCHECK(c, "k_cycle_end");
         }
@@ -663,8 +693,12 @@ int wait_cycle(wl_ctx* c, int target) {
     cudaStream_t gs = proxy ? c->own_stream : user;
     for (unsigned spins = 0;; ++spins) {
         if (hm->cycle >= target) return WL_OK;
+#if defined(__x86_64__) || defined(__i386__)
+        __builtin_ia32_pause();
+#endif
         if ((spins & 0xfff) == 0xfff) {
             cudaError_t e = cudaStreamQuery(gs);
+            if (e == cudaSuccess && gs != user) e = cudaStreamQuery(user);
             if (e == cudaSuccess) {
                 if (hm->cycle >= target) return WL_OK;
                 return fail(c, WL_ECUDA, "wl_solve: the stream drained without recording the cycle");
@@ -699,7 +733,7 @@ int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, dou
                 ++launched;
             }
             if ((rc = wait_cycle(c, known + 1))) return rc;
-            hist[known] = c->h_hist[known];
+            hist[known] = ((volatile double*)c->h_hist)[known];
             nb = hm->nb;
             k = known++;
             if (!(hist[k] > tol * nb) || k >= maxcycles) break;
@@ -727,13 +761,52 @@ int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, dou
             }
             if ((rc = wait_cycle(c, k + 1))) return rc;
             ++k;
-            hist[k] = c->h_hist[k];
+            hist[k] = ((volatile double*)c->h_hist)[k];
             if (!(hist[k] > tol * nb) || k >= maxcycles) stop = true;
         }
         if (k == 0 && (rc = DISPATCH(c, remove_mean)(c, p))) return rc;
     }
     CU(c, cudaStreamSynchronize(c->stream));
     *ncycles = k;
+    return (hist[k] > tol * nb) ? WL_NOT_CONVERGED : WL_OK;
+}
+
+// V-cycle-preconditioned conjugate gradients (oracle: ctx_solve_pcg).  One graph launch per iteration; the stop decision is
+// taken on the device (last CTA of the x/r update) and mirrored to pinned host memory, which the host polls.
+int solve_pcg_impl(wl_ctx* c, void* x, const void* b, double tol, int maxit, double* hist, int* nit, bool have_nb = false) {
+    int rc;
+    if ((rc = ensure_hist(c, maxit))) return rc;
+    const size_t bytes = (size_t)c->lev[0].g.M * c->esz;
+    for (int i = 0; i < 4; ++i)
+        if (!c->cg_v[i]) {
+            if (cudaMalloc(&c->cg_v[i], bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "wl_solve_pcg: cudaMalloc(work vector)"); }
+            drop_graph(c);
+        }
+    if ((rc = DISPATCH(c, prepare)(c))) return rc;
+    if (!have_nb && (rc = DISPATCH(c, absmax_b)(c, b))) return rc;
+    volatile Scalars* hm = c->h_scal;
+    CU(c, cudaStreamSynchronize(c->stream));   // nothing of an earlier call may still write the mirror
+    hm->cycle = 0;
+    hm->done = 0;
+    k_pcg_begin<<<1, 32, 0, c->stream>>>(c->d_scal, tol, maxit);
+    KCHECK(c, "k_pcg_begin");
+    CU(c, cudaMemsetAsync(c->cg_v[2], 0, bytes, c->stream));   // p = 0: the first direction is z itself
+    if ((rc = DISPATCH(c, pcg_residual)(c, x, b))) return rc;
+    int k = 0;
+    double nb = 0.0;
+    while (true) {
+        if ((rc = wait_cycle(c, k + 1))) return rc;
+        if (hm->done == 2) break;                       // breakdown: the residual is exactly 0, no new entry
+        hist[k] = ((volatile double*)c->h_hist)[k];
+        nb = hm->nb;
+        if (!(hist[k] > tol * nb) || k >= maxit) break;
+        if ((rc = run_cycle(c, x, b, true, false, true))) return rc;
+        ++k;
+    }
+    if (hm->done == 2) { --k; if (k < 0) k = 0; }
+    if ((rc = DISPATCH(c, remove_mean)(c, x))) return rc;
+    CU(c, cudaStreamSynchronize(c->stream));
+    *nit = k;
     return (hist[k] > tol * nb) ? WL_NOT_CONVERGED : WL_OK;
 }
 
@@ -862,6 +935,7 @@ void wl_destroy(wl_ctx* c) {
     if (c->h_hist) cudaFreeHost(c->h_hist);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     if (c->b0) cudaFree(c->b0);
+    for (int i = 0; i < 4; ++i) if (c->cg_v[i]) cudaFree(c->cg_v[i]);
     if (c->stage_u) cudaFree(c->stage_u);
     if (c->stage_L) cudaFree(c->stage_L);
     if (c->stage_p) cudaFree(c->stage_p);
@@ -884,6 +958,7 @@ int wl_set_option(wl_ctx* c, int key, int value) {
         case WL_OPT_GRAPH: c->opt_graph = value ? 1 : 0; return WL_OK;
         case WL_OPT_COARSE_CTA: c->opt_coarse_cta = value ? 1 : 0; return WL_OK;
         case WL_OPT_SOLVE_KERNELS: c->opt_solve_kernels = value ? 1 : 0; return WL_OK;
+        case WL_OPT_SOLVER: c->opt_solver = value ? 1 : 0; return WL_OK;
         default: return fail(c, WL_EINVAL, "wl_set_option: unknown key");
     }
 }
@@ -914,6 +989,13 @@ int wl_solve(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, doubl
     return solve_impl(c, p, b, tol, maxcycles, hist, ncycles);
 }
 
+int wl_solve_pcg(wl_ctx* c, void* p, const void* b, double tol, int maxit, double* hist, int* nit) {
+    if (!c) return WL_EINVAL;
+    if (!p || !b || !hist || !nit || maxit < 0 || !(tol >= 0.0)) return fail(c, WL_EINVAL, "wl_solve_pcg: bad argument");
+    if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_solve_pcg: coefficients not set");
+    return solve_pcg_impl(c, p, b, tol, maxit, hist, nit);
+}
+
 int wl_project(wl_ctx* c, void* u, const void* L, void* p, double tol, int maxcycles, double* hist, int* ncycles) {
     if (!c) return WL_EINVAL;
     if (!u || !p || !hist || !ncycles || maxcycles < 0 || !(tol >= 0.0)) return fail(c, WL_EINVAL, "wl_project: bad argument");
@@ -924,7 +1006,8 @@ int wl_project(wl_ctx* c, void* u, const void* L, void* p, double tol, int maxcy
         if (cudaMalloc(&c->b0, (size_t)c->lev[0].g.M * c->esz) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "wl_project: cudaMalloc(b)"); }
     }
     if ((rc = DISPATCH(c, divergence)(c, u, c->b0, true))) return rc;
-    int src = solve_impl(c, p, c->b0, tol, maxcycles, hist, ncycles, true);
+    int src = c->opt_solver ? solve_pcg_impl(c, p, c->b0, tol, maxcycles, hist, ncycles, true)
+                            : solve_impl(c, p, c->b0, tol, maxcycles, hist, ncycles, true);
     if (src < 0) return src;
     if ((rc = DISPATCH(c, gradient)(c, u, p))) return rc;
     CU(c, cudaStreamSynchronize(c->stream));

@@ -28,6 +28,9 @@ struct Scalars {
     int done;                           // 1 once hist[cycle] <= tol * nb
     int maxcycles;
     unsigned int ticket;                // CTAs of the running level-0 launch that have finished (last one does the bookkeeping)
+    double rho, alpha, beta;            // conjugate-gradient scalars (wl_pcg.cuh)
+    int breakdown;                      // rho' = 0 or sigma = 0: the residual is exactly 0
+    int pad;
 };
 
 template <typename T> struct Omega;
