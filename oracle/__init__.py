@@ -50,6 +50,8 @@ def lib():
         L.orc_vcycle.restype, L.orc_vcycle.argtypes = f64, [vp, vp, vp]
         L.orc_solve.restype, L.orc_solve.argtypes = i32, [vp, vp, vp, f64, i32, f64p, i32p]
         L.orc_project.restype, L.orc_project.argtypes = i32, [vp, vp, vp, vp, f64, i32, f64p, i32p]
+        L.orc_mu0.restype, L.orc_mu0.argtypes = f64, [f64]
+        L.orc_body_coeff.restype, L.orc_body_coeff.argtypes = i32, [i32, i64p, i32, i32, f64p, vp]
         L.orc_solve_pcg.restype, L.orc_solve_pcg.argtypes = i32, [vp, vp, vp, f64, i32, f64p, i32p]
         L.orc_divergence.restype, L.orc_divergence.argtypes = None, [vp, vp, vp]
         L.orc_gradient_correct.restype, L.orc_gradient_correct.argtypes = None, [vp, vp, vp]
@@ -60,6 +62,39 @@ def lib():
 
 def _ptr(a: np.ndarray):
     return a.ctypes.data_as(ctypes.c_void_p)
+
+
+BODY_SPHERE, BODY_TORUS = 0, 1
+
+
+def body_records(bodies) -> np.ndarray:
+    """Pack bodies [(kind, centre, R[, r]), ...] into the 8-doubles-per-body records of orc_body_coeff / wl_set_bodies."""
+    rec = np.zeros((len(bodies), 8), dtype=np.float64)
+    for k, bd in enumerate(bodies):
+        kind, centre, R = bd[0], bd[1], bd[2]
+        rec[k, 0] = kind
+        rec[k, 1:1 + len(centre)] = centre
+        rec[k, 4] = R
+        rec[k, 5] = bd[3] if len(bd) > 3 else 0.0
+    return rec
+
+
+def mu0(d: float) -> float:
+    return float(lib().orc_mu0(float(d)))
+
+
+def body_coeff(dims, dtype, bodies) -> np.ndarray:
+    """BDIM face coefficients L = mu0(min_k d_k) at the face centres (NEXT-3), walls zeroed; shape (n, N_{n-1}, ..., N_0)."""
+    dims = tuple(int(d) for d in dims)
+    n = len(dims)
+    dt = np.dtype(dtype)
+    rec = np.ascontiguousarray(bodies, dtype=np.float64).reshape(-1, 8)
+    out = np.empty((n,) + tuple(reversed(dims)), dtype=dt)
+    arr = (ctypes.c_int64 * n)(*dims)
+    rc = lib().orc_body_coeff(n, arr, 0 if dt == np.float32 else 1, rec.shape[0],
+                              rec.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), _ptr(out))
+    assert rc == 0
+    return out
 
 
 class Oracle:

@@ -35,11 +35,18 @@
 //                  DESIGN.md section 3 reading 13: the paper gives no detail -> "parity unpinned" by any
 //                  value of the paper.
 //
+//   body_coeff     (the BDIM! row of Table 2)
+//                  pinned: mu0(-1) = 0, mu0(0) = 1/2, mu0(1) = 1, mu0(d) + mu0(-d) = 1, monotone, C^1 at
+//                  +-1 (derivative 0); exact 0 / 1 at faces farther than one cell inside / outside a body;
+//                  the cell-integral of 1 - L over a sphere reproduces its volume; face-centre
+//                  convention checked on a half-space-like huge sphere (tests/test_oracle_body.py).
+//
 // Notation: n = ndim in {2,3}; N = (N_0..N_{n-1}), axis 0 unit-stride; cell I has
 // linear index I_0 + N_0 (I_1 + N_1 I_2); face (I,i) is the LOWER face of cell I in direction i
 // (coeff[I,i] multiplies p[I]-p[I-del(i)]).  L, u are n cell-sized fields back to
 // back (component slowest).  The upper wall face I_i = N_i is not stored and has L = 0, u = 0.
 
+#define _USE_MATH_DEFINES
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -465,6 +472,54 @@ int ctx_project(Ctx<T>* c, T* u, const T* L, T* p, double tol, int maxcycles, do
     return rc;
 }
 
+// ---------------------------------------------------------------------------------------------
+// BDIM coefficients from analytic bodies (NEXT-3).  BJ "BDIM face coefficient L = mu0(d): 0 for
+// d <= -1, 1 for d >= 1, otherwise 0.5(1 + d + sin(pi d)/pi), where d is the signed distance to the
+// body in cells, taken at the face centre and positive in the fluid."  Several bodies: d = min.
+// Evaluated in fp64, clamped to [0,1], then cast (c-8); face (I,i) has coordinate I_i along i and
+// I_j + 1/2 along the other axes (c-9); the stored wall plane I_i = 0 is 0 (c-6).
+// Body record (8 doubles): kind (0 sphere / circle, 1 torus about axis 0), c0, c1, c2, R, r, -, -.
+// ---------------------------------------------------------------------------------------------
+double mu0(double d) {
+    if (d <= -1.0) return 0.0;
+    if (d >= 1.0) return 1.0;
+    double v = 0.5 * (1.0 + d + std::sin(M_PI * d) / M_PI);
+    if (v < 0.0) v = 0.0;
+    if (v > 1.0) v = 1.0;
+    return v;
+}
+
+double body_distance(int n, const double* B, const double* x) {
+    const double dx = x[0] - B[1], dy = x[1] - B[2], dz = (n > 2) ? x[2] - B[3] : 0.0;
+    if ((int)B[0] == 0) {
+        double r2 = dx * dx + dy * dy;
+        if (n > 2) r2 = r2 + dz * dz;
+        return std::sqrt(r2) - B[4];
+    }
+    const double rho = std::sqrt(dy * dy + dz * dz) - B[4];
+    return std::sqrt(rho * rho + dx * dx) - B[5];
+}
+
+template <class T>
+void body_coeff(const Dims& g, int nbodies, const double* bodies, T* L) {
+    for (int i = 0; i < g.n; ++i)
+        for (int64_t I2 = 0; I2 < g.N[2]; ++I2)
+            for (int64_t I1 = 0; I1 < g.N[1]; ++I1)
+                for (int64_t I0 = 0; I0 < g.N[0]; ++I0) {
+                    const int64_t Ii[3] = {I0, I1, I2};
+                    const int64_t e = (int64_t)i * g.M + I0 + g.N[0] * (I1 + g.N[1] * I2);
+                    if (Ii[i] == 0) { L[e] = (T)0; continue; }
+                    double x[3];
+                    for (int j = 0; j < 3; ++j) x[j] = (double)Ii[j] + ((j == i) ? 0.0 : 0.5);
+                    double d = 1.0e300;
+                    for (int k = 0; k < nbodies; ++k) {
+                        const double dk = body_distance(g.n, bodies + 8 * k, x);
+                        if (dk < d) d = dk;
+                    }
+                    L[e] = (T)mu0(d);
+                }
+}
+
 struct Handle {
     int dtype;  // 0 = f32, 1 = f64
     void* ctx;
@@ -577,6 +632,16 @@ int orc_solve(void* hv, void* p, const void* b, double tol, int maxcycles, doubl
     DISPATCH(h, rc = ctx_solve(c, (T*)p, (const T*)b, tol, maxcycles, hist, ncycles),
                 rc = ctx_solve(c, (T*)p, (const T*)b, tol, maxcycles, hist, ncycles));
     return rc;
+}
+
+double orc_mu0(double d) { return mu0(d); }
+
+// L (n*M elements of dtype) for `nbodies` bodies on a grid of `dims`
+int orc_body_coeff(int ndim, const int64_t* dims, int dtype, int nbodies, const double* bodies, void* L) {
+    if (ndim < 2 || ndim > 3) return -1;
+    Dims g = make_dims(ndim, dims);
+    if (dtype == 0) body_coeff(g, nbodies, bodies, (float*)L); else body_coeff(g, nbodies, bodies, (double*)L);
+    return 0;
 }
 
 int orc_solve_pcg(void* hv, void* p, const void* b, double tol, int maxit, double* hist, int* nit) {

@@ -29,6 +29,7 @@ SIGNATURES = {
     "wl_set_stream": (_i32, [_vp, _vp]),
     "wl_set_option": (_i32, [_vp, _i32, _i32]),
     "wl_set_coeff": (_i32, [_vp, _vp]),
+    "wl_set_bodies": (_i32, [_vp, _i32, _f64p]),
     "wl_vcycle": (_i32, [_vp, _vp, _vp, _f64p]),
     "wl_solve": (_i32, [_vp, _vp, _vp, _f64, _i32, _f64p, _i32p]),
     "wl_solve_pcg": (_i32, [_vp, _vp, _vp, _f64, _i32, _f64p, _i32p]),
@@ -128,6 +129,16 @@ def wl_set_option(ctx, key: int, value: int):
 
 def wl_set_coeff(ctx, L):
     return _check(ctx, load().wl_set_coeff(ctx, _dptr(L)), "wl_set_coeff")
+
+
+WL_BODY_SPHERE, WL_BODY_TORUS = 0, 1
+
+
+def wl_set_bodies(ctx, records):
+    """records: array-like (nbodies, 8) of float64: kind, c0, c1, c2, R, r, 0, 0 (see include/wl.h)."""
+    rec = np.ascontiguousarray(records, dtype=np.float64).reshape(-1, 8)
+    ptr = rec.ctypes.data_as(_f64p) if rec.shape[0] else None
+    return _check(ctx, load().wl_set_bodies(ctx, int(rec.shape[0]), ptr), "wl_set_bodies")
 
 
 def wl_vcycle(ctx, p, b, want_norm: bool = True):

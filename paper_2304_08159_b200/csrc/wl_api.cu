@@ -17,6 +17,7 @@
 #include "wl_tail.cuh"
 #include "wl_rows.cuh"
 #include "wl_pcg.cuh"
+#include "wl_body.cuh"
 
 using namespace wl;
 
@@ -52,6 +53,7 @@ struct wl_ctx {
     double* h_hist = nullptr;    // pinned
     int hist_cap = 0;
     void* b0 = nullptr;          // ctx-owned right-hand side for wl_project
+    double* d_bodies = nullptr;  // device copy of the body records of wl_set_bodies
     void* cg_v[4] = {nullptr, nullptr, nullptr, nullptr};   // r, z, p, q of the conjugate-gradient solve (allocated on first use)
     int opt_solver = 0;          // WL_OPT_SOLVER: 0 = V-cycles (BJ), 1 = V-cycle-preconditioned CG (NEXT-1)
     void* stage_u = nullptr;     // device staging for wl_project_host
@@ -136,6 +138,24 @@ struct Impl {
             k_copy_coeff<T, ND><<<grid_for(c, f.g.M * ND), kBlock, 0, c->stream>>>(f.g, P(Ldev), P(f.L));
             KCHECK(c, "k_copy_coeff");
         }
+        return finish_coeff(c);
+    }
+
+    // NEXT-3: level-0 coefficients from analytic bodies, evaluated on the device (wl_body.cuh), then the same chain.
+    static int set_bodies(wl_ctx* c, int nbodies) {
+        Level& f = c->lev[0];
+        if (rows_ok(f.g, f.L)) {
+            k_body_coeff_rows<T, ND><<<rows_grid(c, (long long)f.g.N1 * f.g.N2 * ND), dim3(kRowsX, kRowsY), 0, c->stream>>>(f.g, c->d_bodies, nbodies, P(f.L));
+            KCHECK(c, "k_body_coeff_rows");
+        } else {
+            k_body_coeff<T, ND><<<grid_for(c, f.g.M * ND), kBlock, 0, c->stream>>>(f.g, c->d_bodies, nbodies, P(f.L));
+            KCHECK(c, "k_body_coeff");
+        }
+        return finish_coeff(c);
+    }
+
+    // coarsening chain (one kernel per level, fixed summation tree) and omega/D per level
+    static int finish_coeff(wl_ctx* c) {
         for (int l = 0; l + 1 < c->nlev; ++l) {
             Level& a = c->lev[l];
             Level& b = c->lev[l + 1];
@@ -935,6 +955,7 @@ void wl_destroy(wl_ctx* c) {
     if (c->h_hist) cudaFreeHost(c->h_hist);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     if (c->b0) cudaFree(c->b0);
+    if (c->d_bodies) cudaFree(c->d_bodies);
     for (int i = 0; i < 4; ++i) if (c->cg_v[i]) cudaFree(c->cg_v[i]);
     if (c->stage_u) cudaFree(c->stage_u);
     if (c->stage_L) cudaFree(c->stage_L);
@@ -967,6 +988,24 @@ int wl_set_coeff(wl_ctx* c, const void* L) {
     if (!c) return WL_EINVAL;
     if (!L) return fail(c, WL_EINVAL, "wl_set_coeff: null L");
     return DISPATCH(c, set_coeff)(c, L);
+}
+
+int wl_set_bodies(wl_ctx* c, int nbodies, const double* bodies_host) {
+    if (!c) return WL_EINVAL;
+    if (nbodies < 0 || nbodies > kMaxBodies || (nbodies > 0 && !bodies_host)) return fail(c, WL_EINVAL, "wl_set_bodies: bad argument (at most 256 bodies)");
+    for (int k = 0; k < nbodies; ++k) {
+        const double* B = bodies_host + (size_t)k * kBodyDoubles;
+        const int kind = (int)B[0];
+        if ((kind != WL_BODY_SPHERE && kind != WL_BODY_TORUS) || (kind == WL_BODY_TORUS && c->n != 3) || !(B[4] >= 0.0) || !(B[5] >= 0.0))
+            return fail(c, WL_EINVAL, "wl_set_bodies: bad body record");
+    }
+    if (!c->d_bodies && cudaMalloc((void**)&c->d_bodies, sizeof(double) * kMaxBodies * kBodyDoubles) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, WL_ENOMEM, "wl_set_bodies: cudaMalloc");
+    }
+    if (nbodies > 0)   // pageable host memory: the copy is staged before the call returns, the caller's array may be reused
+        CU(c, cudaMemcpyAsync(c->d_bodies, bodies_host, sizeof(double) * (size_t)nbodies * kBodyDoubles, cudaMemcpyHostToDevice, c->stream));
+    return DISPATCH(c, set_bodies)(c, nbodies);
 }
 
 int wl_vcycle(wl_ctx* c, void* p, const void* b, double* rnorm_out) {
