@@ -205,6 +205,7 @@ def main():
     ap.add_argument("--dtype", default=None, choices=[None, "float32", "float64"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-upload-L", action="store_true", help="e2e leg: upload the n·M coefficient array instead of the body records")
     ap.add_argument("--no-pcg", action="store_true", help="skip the conjugate-gradient leg (reported beside the V-cycle solver)")
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--graph", type=int, default=1)
@@ -278,23 +279,56 @@ def main():
         barrier()
         total_ms = float(np.sum(ms))
 
-        # e2e: same projection through the host-buffer entry point (H2D u, L, p; D2H u, p inside the timed region)
+        # the dominant kernels alone (roofline leg), straight after the timed steps
+        kern = {}
+        reps = max(5, args.kernel_reps)
+        if pr.num_levels > 1:
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 1)   # time the instances the solve's graph launches
+            bd = pr.empty_cells()
+            wl.wl_divergence(pr.ctx, u0, bd)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            xo = pr.empty_cells()
+            for name, fn in (("down", lambda: wl.wl_down(pr.ctx, 0, p, bd, xo)),
+                             ("up", lambda: wl.wl_up(pr.ctx, 0, xo, None, bd, p))):
+                for _ in range(3):
+                    fn()
+                l0 = wl.wl_launch_count(pr.ctx)
+                torch.cuda.synchronize()
+                e0.record(stream)
+                for _ in range(reps):
+                    fn()
+                e1.record(stream)
+                e1.synchronize()
+                kern[name] = {"ms": e0.elapsed_time(e1) / reps, "launches_per_call": (wl.wl_launch_count(pr.ctx) - l0) // reps}
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 0)
+            del xo
+
+        # e2e: the same projection through the host-buffer entry point with pinned HOST buffers.  Inputs of a step: the
+        # face velocity u (n·M values) and the bodies' analytic description (8 doubles each) from which wl_set_bodies builds
+        # the coefficient hierarchy on the device (no coefficient array crosses the bus); p starts from 0
+        # (WL_OPT_HOST_P_ZERO).  Results read back every step: u and p.  --e2e-upload-L uploads the n·M coefficients instead.
         if not args.no_e2e:
             uh = torch.empty_like(u_host).pin_memory()
             ph = torch.zeros(pr.cell_shape(), dtype=pr.torch_dtype).pin_memory()
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_HOST_P_ZERO, 1)
             e2e_ms = []
             for it in range(2 + args.steps):
                 uh.copy_(u_host)
-                ph.zero_()
                 torch.cuda.synchronize()
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
-                h2, nc2, rc2 = wl.wl_project_host(pr.ctx, uh, L_host, ph, tol, maxc)
+                if args.e2e_upload_L:
+                    h2, nc2, rc2 = wl.wl_project_host(pr.ctx, uh, L_host, ph, tol, maxc)
+                else:
+                    wl.wl_set_bodies(pr.ctx, cfg["bodies"])
+                    h2, nc2, rc2 = wl.wl_project_host(pr.ctx, uh, None, ph, tol, maxc)
                 e1.record(stream)
                 e1.synchronize()
                 if it >= 2:
                     e2e_ms.append(e0.elapsed_time(e1))
             e2e_total = float(np.sum(e2e_ms))
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_HOST_P_ZERO, 0)
+            wl.wl_set_coeff(pr.ctx, Ld)   # back to the uploaded field for the legs below
 
         # NEXT-1 beside the specified solver: the same projection with V-cycle-preconditioned conjugate gradients
         pcg = None
@@ -311,9 +345,9 @@ def main():
 
         # V-cycles alone: wl_solve with tol = 0 runs exactly `reps` cycles (one graph launch + one 8-byte readback each,
         # mean shift deferred into the next cycle); the dominant kernels alone follow
-        bd = pr.empty_cells()
-        wl.wl_divergence(pr.ctx, u0, bd)
-        reps = max(5, args.kernel_reps)
+        if pr.num_levels <= 1:
+            bd = pr.empty_cells()
+            wl.wl_divergence(pr.ctx, u0, bd)
         p.zero_()
         wl.wl_solve(pr.ctx, p, bd, 0.0, 3)
         p.zero_()
@@ -325,22 +359,6 @@ def main():
         e1.synchronize()
         vcycle_ms = e0.elapsed_time(e1) / reps
 
-        kern = {}
-        if pr.num_levels > 1:
-            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 1)   # time the instances the solve's graph launches
-            xo = pr.empty_cells()
-            for name, fn in (("down", lambda: wl.wl_down(pr.ctx, 0, p, bd, xo)),
-                             ("up", lambda: wl.wl_up(pr.ctx, 0, xo, None, bd, p))):
-                for _ in range(3):
-                    fn()
-                l0 = wl.wl_launch_count(pr.ctx)
-                torch.cuda.synchronize()
-                e0.record(stream)
-                for _ in range(reps):
-                    fn()
-                e1.record(stream)
-                e1.synchronize()
-                kern[name] = {"ms": e0.elapsed_time(e1) / reps, "launches_per_call": (wl.wl_launch_count(pr.ctx) - l0) // reps}
     clocks = clk.summary()
 
     # max over ranks
@@ -390,10 +408,12 @@ def main():
     }
     if not args.no_e2e:
         e2e_sec = e2e_total / 1e3 / args.steps
-        h2d = u_host.numel() * esz + L_host.numel() * esz + M * esz
+        h2d = u_host.numel() * esz + (L_host.numel() * esz if args.e2e_upload_L else int(cfg["bodies"].size) * 8)
         d2h = u_host.numel() * esz + M * esz
         line["e2e"] = {"value": whole_job_value(world, M, int(nc2), e2e_sec), "unit": UNIT, "ms_per_step": e2e_sec * 1e3,
-                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
+                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "cycles_run": int(nc2),
+                       "inputs": "u + coefficient array L (wl_set_coeff inside wl_project_host)" if args.e2e_upload_L
+                                 else "u + body records (wl_set_bodies builds L on the device); p0 = 0 not uploaded"}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         # the oracle as it stands, one thread, bounded sample: one V-cycle of the same workload

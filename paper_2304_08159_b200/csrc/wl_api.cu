@@ -6,6 +6,8 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <string.h>
+#include <initializer_list>
+#include <math.h>
 #include <new>
 #include <vector>
 
@@ -59,17 +61,26 @@ struct wl_ctx {
     void* stage_u = nullptr;     // device staging for wl_project_host
     void* stage_L = nullptr;
     void* stage_p = nullptr;
+    cudaStream_t copy_stream = nullptr;   // wl_project_host: copies that overlap kernels of the ctx stream
+    cudaEvent_t ev_copy[3] = {nullptr, nullptr, nullptr};
+    int opt_host_p_zero = 0;     // WL_OPT_HOST_P_ZERO: wl_project_host starts from p = 0 without uploading p_host
     bool have_coeff = false;
     int opt_fused = 1, opt_graph = 1, opt_coarse_cta = 1, opt_solve_kernels = 0;
     int num_sms = 148;
     // cached CUDA graph of one V-cycle (H9), valid for one (p, b, variant, stream, options) combination
     cudaStream_t own_stream = nullptr;   // the legacy default stream cannot be captured: graphs then run here, fenced by events
     cudaEvent_t ev_in = nullptr, ev_out = nullptr;
-    cudaGraphExec_t cg_exec = nullptr;
-    void* cg_p = nullptr;
-    const void* cg_b = nullptr;
-    int cg_variant = -1;
-    int64_t cg_nodes = 0;
+    struct GraphEntry {          // a small LRU: a time stepper that alternates two pressure buffers, or mixes wl_vcycle with
+        cudaGraphExec_t exec = nullptr;   // wl_solve, does not re-capture on every call
+        void* p = nullptr;
+        const void* b = nullptr;
+        int variant = -1;
+        int64_t nodes = 0;
+        uint64_t stamp = 0;
+    } cg[4];
+    uint64_t cg_clock = 0;
+    bool unaligned = false;      // a caller array of the running call is not 16-byte aligned: no TMA on its level
+    int unaligned_level = 0;
     int tail_first = kMaxLevels; // first level of the single-CTA coarse tail (>= nlev: none fits shared memory)
     int check_done = 0;          // set while enqueuing a solve cycle: kernels that can, return at once when scal->done
     int fused_grid = 0;          // CTAs of the last fused launch (= number of sum partials it wrote)
@@ -263,6 +274,7 @@ struct Impl {
 
     static bool fused_ok(const wl_ctx* c, int l) {
         if (!c->opt_fused || l + 1 >= c->nlev) return false;
+        if (c->unaligned && l == c->unaligned_level) return false;   // TMA needs 16-byte aligned arrays: generic kernels instead
         const Grid& g = c->lev[l].g;
         constexpr int VEC = 16 / (int)sizeof(T);
         if (g.N0 % (2 * VEC)) return false;
@@ -647,9 +659,10 @@ int ensure_hist(wl_ctx* c, int maxcycles) {
 }
 
 void drop_graph(wl_ctx* c) {
-    if (c->cg_exec) cudaGraphExecDestroy(c->cg_exec);
-    c->cg_exec = nullptr;
-    c->cg_variant = -1;
+    for (auto& e : c->cg) {
+        if (e.exec) cudaGraphExecDestroy(e.exec);
+        e = wl_ctx::GraphEntry();
+    }
 }
 
 // One V-cycle (+ k_cycle_end bookkeeping when `in_solve`) on the ctx stream: a cached CUDA graph when WL_OPT_GRAPH is on.
@@ -672,8 +685,15 @@ int run_cycle(wl_ctx* c, void* p, const void* b, bool in_solve, bool lagged, boo
     cudaStream_t user = c->stream;
     const bool proxy = (user == nullptr || user == cudaStreamLegacy || user == cudaStreamPerThread);
     cudaStream_t gs = proxy ? c->own_stream : user;
-    if (!(c->cg_exec && c->cg_p == p && c->cg_b == b && c->cg_variant == variant)) {
-        drop_graph(c);
+    wl_ctx::GraphEntry* ge = nullptr;
+    for (auto& e : c->cg)
+        if (e.exec && e.p == p && e.b == b && e.variant == variant) ge = &e;
+    if (!ge) {
+        ge = &c->cg[0];
+        for (auto& e : c->cg)                       // a free entry, else the least recently used one
+            if (!e.exec || (ge->exec && e.stamp < ge->stamp)) { ge = &e; if (!e.exec) break; }
+        if (ge->exec) cudaGraphExecDestroy(ge->exec);
+        *ge = wl_ctx::GraphEntry();
         if ((rc = DISPATCH(c, prepare)(c))) return rc;
         const int64_t before = c->launches;
         CU(c, cudaStreamBeginCapture(gs, cudaStreamCaptureModeThreadLocal));
@@ -682,25 +702,26 @@ int run_cycle(wl_ctx* c, void* p, const void* b, bool in_solve, bool lagged, boo
         c->stream = user;
         cudaGraph_t graph = nullptr;
         cudaError_t e = cudaStreamEndCapture(gs, &graph);
-        c->cg_nodes = c->launches - before;
+        ge->nodes = c->launches - before;
         c->launches = before;
         if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
         if (e != cudaSuccess) return fail(c, WL_ECUDA, "cudaStreamEndCapture", e);
-        e = cudaGraphInstantiate(&c->cg_exec, graph, 0);
+        e = cudaGraphInstantiate(&ge->exec, graph, 0);
         cudaGraphDestroy(graph);
-        if (e != cudaSuccess) { c->cg_exec = nullptr; return fail(c, WL_ECUDA, "cudaGraphInstantiate", e); }
-        c->cg_p = p; c->cg_b = b; c->cg_variant = variant;
+        if (e != cudaSuccess) { ge->exec = nullptr; return fail(c, WL_ECUDA, "cudaGraphInstantiate", e); }
+        ge->p = p; ge->b = b; ge->variant = variant;
     }
+    ge->stamp = ++c->cg_clock;
     if (proxy) {
         CU(c, cudaEventRecord(c->ev_in, user));
         CU(c, cudaStreamWaitEvent(gs, c->ev_in, 0));
     }
-    CU(c, cudaGraphLaunch(c->cg_exec, gs));
+    CU(c, cudaGraphLaunch(ge->exec, gs));
     if (proxy) {
         CU(c, cudaEventRecord(c->ev_out, gs));
         CU(c, cudaStreamWaitEvent(user, c->ev_out, 0));
     }
-    c->launches += c->cg_nodes;
+    c->launches += ge->nodes;
     return WL_OK;
 }
 
@@ -788,6 +809,7 @@ int solve_impl(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, dou
     }
     CU(c, cudaStreamSynchronize(c->stream));
     *ncycles = k;
+    if (!isfinite(hist[k]) || !isfinite(nb)) return fail(c, WL_ENONFINITE, "wl_solve: the residual norm is not finite (NaN or Inf in p, b or the coefficients)");
     return (hist[k] > tol * nb) ? WL_NOT_CONVERGED : WL_OK;
 }
 
@@ -827,7 +849,17 @@ int solve_pcg_impl(wl_ctx* c, void* x, const void* b, double tol, int maxit, dou
     if ((rc = DISPATCH(c, remove_mean)(c, x))) return rc;
     CU(c, cudaStreamSynchronize(c->stream));
     *nit = k;
+    if (!isfinite(hist[k]) || !isfinite(nb)) return fail(c, WL_ENONFINITE, "wl_solve_pcg: the residual norm is not finite (NaN or Inf in p, b or the coefficients)");
     return (hist[k] > tol * nb) ? WL_NOT_CONVERGED : WL_OK;
+}
+
+// Fused (TMA) kernels need 16-byte aligned arrays; a misaligned caller array (e.g. a torch slice) sends its level to the
+// generic kernels instead of failing in cuTensorMapEncodeTiled.
+void note_alignment(wl_ctx* c, int level, std::initializer_list<const void*> ptrs) {
+    uintptr_t bits = 0;
+    for (const void* q : ptrs) bits |= (uintptr_t)q;
+    c->unaligned = (bits & 15) != 0;
+    c->unaligned_level = level;
 }
 
 int level_check(const wl_ctx* c, int level, bool need_next) {
@@ -911,17 +943,20 @@ int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
         okm = false;
         snprintf(g_create_err, sizeof(g_create_err), "wl_create: cudaMallocHost failed");
     }
-    if (okm && cudaMemset(c->d_scal, 0, sizeof(Scalars)) != cudaSuccess) okm = false;
-    if (okm && (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
-                cudaEventCreateWithFlags(&c->ev_in, cudaEventDisableTiming) != cudaSuccess ||
-                cudaEventCreateWithFlags(&c->ev_out, cudaEventDisableTiming) != cudaSuccess)) {
-        okm = false;
-        snprintf(g_create_err, sizeof(g_create_err), "wl_create: stream/event creation failed");
-    }
     if (!okm) {
         cudaGetLastError();
         wl_destroy(c);
         return WL_ENOMEM;
+    }
+    cudaError_t e3 = cudaMemset(c->d_scal, 0, sizeof(Scalars));
+    if (e3 == cudaSuccess) e3 = cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking);
+    if (e3 == cudaSuccess) e3 = cudaEventCreateWithFlags(&c->ev_in, cudaEventDisableTiming);
+    if (e3 == cudaSuccess) e3 = cudaEventCreateWithFlags(&c->ev_out, cudaEventDisableTiming);
+    if (e3 != cudaSuccess) {   // not an allocation failure
+        snprintf(g_create_err, sizeof(g_create_err), "wl_create: stream / event / memset: %s", cudaGetErrorString(e3));
+        cudaGetLastError();
+        wl_destroy(c);
+        return WL_ECUDA;
     }
     if (DISPATCH(c, init_kernels)(c) != WL_OK) {
         snprintf(g_create_err, sizeof(g_create_err), "wl_create: %s", c->err);
@@ -938,6 +973,8 @@ void wl_destroy(wl_ctx* c) {
     cudaStreamSynchronize(c->stream);
     drop_graph(c);
     if (c->own_stream) { cudaStreamSynchronize(c->own_stream); cudaStreamDestroy(c->own_stream); }
+    if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
+    for (int i = 0; i < 3; ++i) if (c->ev_copy[i]) cudaEventDestroy(c->ev_copy[i]);
     if (c->ev_in) cudaEventDestroy(c->ev_in);
     if (c->ev_out) cudaEventDestroy(c->ev_out);
     for (int l = 0; l < kMaxLevels; ++l) {
@@ -980,6 +1017,7 @@ int wl_set_option(wl_ctx* c, int key, int value) {
         case WL_OPT_COARSE_CTA: c->opt_coarse_cta = value ? 1 : 0; return WL_OK;
         case WL_OPT_SOLVE_KERNELS: c->opt_solve_kernels = value ? 1 : 0; return WL_OK;
         case WL_OPT_SOLVER: c->opt_solver = value ? 1 : 0; return WL_OK;
+        case WL_OPT_HOST_P_ZERO: c->opt_host_p_zero = value ? 1 : 0; return WL_OK;
         default: return fail(c, WL_EINVAL, "wl_set_option: unknown key");
     }
 }
@@ -1012,6 +1050,7 @@ int wl_vcycle(wl_ctx* c, void* p, const void* b, double* rnorm_out) {
     if (!c) return WL_EINVAL;
     if (!p || !b) return fail(c, WL_EINVAL, "wl_vcycle: null pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle: coefficients not set");
+    note_alignment(c, 0, {p, b});
     int rc = run_cycle(c, p, b, false, false);
     if (rc) return rc;
     if (rnorm_out) {
@@ -1025,6 +1064,7 @@ int wl_solve(wl_ctx* c, void* p, const void* b, double tol, int maxcycles, doubl
     if (!c) return WL_EINVAL;
     if (!p || !b || !hist || !ncycles || maxcycles < 0 || !(tol >= 0.0)) return fail(c, WL_EINVAL, "wl_solve: bad argument");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_solve: coefficients not set");
+    note_alignment(c, 0, {p, b});
     return solve_impl(c, p, b, tol, maxcycles, hist, ncycles);
 }
 
@@ -1032,6 +1072,7 @@ int wl_solve_pcg(wl_ctx* c, void* p, const void* b, double tol, int maxit, doubl
     if (!c) return WL_EINVAL;
     if (!p || !b || !hist || !nit || maxit < 0 || !(tol >= 0.0)) return fail(c, WL_EINVAL, "wl_solve_pcg: bad argument");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_solve_pcg: coefficients not set");
+    note_alignment(c, 0, {p, b});
     return solve_pcg_impl(c, p, b, tol, maxit, hist, nit);
 }
 
@@ -1044,6 +1085,7 @@ int wl_project(wl_ctx* c, void* u, const void* L, void* p, double tol, int maxcy
     if (!c->b0) {
         if (cudaMalloc(&c->b0, (size_t)c->lev[0].g.M * c->esz) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "wl_project: cudaMalloc(b)"); }
     }
+    note_alignment(c, 0, {p});
     if ((rc = DISPATCH(c, divergence)(c, u, c->b0, true))) return rc;
     int src = c->opt_solver ? solve_pcg_impl(c, p, c->b0, tol, maxcycles, hist, ncycles, true)
                             : solve_impl(c, p, c->b0, tol, maxcycles, hist, ncycles, true);
@@ -1056,20 +1098,48 @@ int wl_project(wl_ctx* c, void* u, const void* L, void* p, double tol, int maxcy
 int wl_project_host(wl_ctx* c, void* u_host, const void* L_host, void* p_host, double tol, int maxcycles, double* hist,
                     int* ncycles) {
     if (!c) return WL_EINVAL;
-    if (!u_host || !p_host || !hist || !ncycles) return fail(c, WL_EINVAL, "wl_project_host: null pointer");
+    if (!u_host || !p_host || !hist || !ncycles || maxcycles < 0 || !(tol >= 0.0)) return fail(c, WL_EINVAL, "wl_project_host: bad argument");
+    if (!L_host && !c->have_coeff) return fail(c, WL_ESTATE, "wl_project_host: coefficients not set");
     const size_t cell_bytes = (size_t)c->lev[0].g.M * c->esz;
     const size_t face_bytes = cell_bytes * c->n;
     if (!c->stage_u && cudaMalloc(&c->stage_u, face_bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "cudaMalloc(stage_u)"); }
     if (!c->stage_p && cudaMalloc(&c->stage_p, cell_bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "cudaMalloc(stage_p)"); }
     if (L_host && !c->stage_L && cudaMalloc(&c->stage_L, face_bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "cudaMalloc(stage_L)"); }
-    CU(c, cudaMemcpyAsync(c->stage_u, u_host, face_bytes, cudaMemcpyHostToDevice, c->stream));
-    CU(c, cudaMemcpyAsync(c->stage_p, p_host, cell_bytes, cudaMemcpyHostToDevice, c->stream));
-    if (L_host) CU(c, cudaMemcpyAsync(c->stage_L, L_host, face_bytes, cudaMemcpyHostToDevice, c->stream));
-    int src = wl_project(c, c->stage_u, L_host ? c->stage_L : nullptr, c->stage_p, tol, maxcycles, hist, ncycles);
+    if (!c->b0 && cudaMalloc(&c->b0, cell_bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "cudaMalloc(b)"); }
+    if (!c->copy_stream) {
+        if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_copy[0], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_copy[1], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_copy[2], cudaEventDisableTiming) != cudaSuccess)
+            return fail(c, WL_ECUDA, "wl_project_host: stream / event creation", cudaGetLastError());
+    }
+    cudaStream_t ms = c->stream, cs = c->copy_stream;
+    int rc;
+    // The copies that nothing waits for yet run on a second stream: L goes first and its hierarchy (H0) is built while u is
+    // still crossing the bus; the pressure leaves while the gradient kernel runs.  One cudaMemcpyAsync per array.
+    CU(c, cudaEventRecord(c->ev_copy[0], ms));                 // earlier work on the ctx stream may still use the staging buffers
+    CU(c, cudaStreamWaitEvent(cs, c->ev_copy[0], 0));
+    if (L_host) {
+        CU(c, cudaMemcpyAsync(c->stage_L, L_host, face_bytes, cudaMemcpyHostToDevice, ms));
+        if ((rc = DISPATCH(c, set_coeff)(c, c->stage_L))) return rc;
+    }
+    CU(c, cudaMemcpyAsync(c->stage_u, u_host, face_bytes, cudaMemcpyHostToDevice, cs));
+    if (c->opt_host_p_zero) CU(c, cudaMemsetAsync(c->stage_p, 0, cell_bytes, cs));
+    else CU(c, cudaMemcpyAsync(c->stage_p, p_host, cell_bytes, cudaMemcpyHostToDevice, cs));
+    CU(c, cudaEventRecord(c->ev_copy[1], cs));
+    CU(c, cudaStreamWaitEvent(ms, c->ev_copy[1], 0));
+    note_alignment(c, 0, {c->stage_p});
+    if ((rc = DISPATCH(c, divergence)(c, c->stage_u, c->b0, true))) return rc;
+    int src = c->opt_solver ? solve_pcg_impl(c, c->stage_p, c->b0, tol, maxcycles, hist, ncycles, true)
+                            : solve_impl(c, c->stage_p, c->b0, tol, maxcycles, hist, ncycles, true);
     if (src < 0) return src;
-    CU(c, cudaMemcpyAsync(u_host, c->stage_u, face_bytes, cudaMemcpyDeviceToHost, c->stream));
-    CU(c, cudaMemcpyAsync(p_host, c->stage_p, cell_bytes, cudaMemcpyDeviceToHost, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
+    CU(c, cudaEventRecord(c->ev_copy[2], ms));                 // p is final
+    CU(c, cudaStreamWaitEvent(cs, c->ev_copy[2], 0));
+    CU(c, cudaMemcpyAsync(p_host, c->stage_p, cell_bytes, cudaMemcpyDeviceToHost, cs));
+    if ((rc = DISPATCH(c, gradient)(c, c->stage_u, c->stage_p))) return rc;
+    CU(c, cudaMemcpyAsync(u_host, c->stage_u, face_bytes, cudaMemcpyDeviceToHost, ms));
+    CU(c, cudaStreamSynchronize(ms));
+    CU(c, cudaStreamSynchronize(cs));
     return src;
 }
 
@@ -1111,6 +1181,7 @@ int wl_down(wl_ctx* c, int level, const void* x_in, const void* b, void* x_out, 
     if (!b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_down: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_down: coefficients not set");
     if (c->opt_solve_kernels) { int rc = ensure_hist(c, 63); if (rc) return rc; }
+    note_alignment(c, level, {x_in, b, x_out, bc});
     return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
 }
 
@@ -1119,6 +1190,7 @@ int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b,
     if (!x_in || !b || !x_out || x_in == x_out) return fail(c, WL_EINVAL, "wl_up: bad pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_up: coefficients not set");
     if (c->opt_solve_kernels) { int rc = ensure_hist(c, 63); if (rc) return rc; }
+    note_alignment(c, level, {x_in, xc, b, x_out});
     return DISPATCH(c, up)(c, level, x_in, xc ? xc : c->lev[level + 1].x[1], b, x_out);
 }
 
@@ -1126,6 +1198,7 @@ int wl_vcycle_level(wl_ctx* c, int level, void* x, const void* b) {
     if (level_check(c, level, false)) return c ? fail(c, WL_EINVAL, "wl_vcycle_level: bad level") : WL_EINVAL;
     if (!x || !b) return fail(c, WL_EINVAL, "wl_vcycle_level: null pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle_level: coefficients not set");
+    note_alignment(c, level, {x, b});
     return DISPATCH(c, vcycle)(c, level, x, b, level == 0 ? c->lev[0].x[1] : c->lev[level].x[0], x);
 }
 

@@ -37,11 +37,14 @@ template <typename T> struct Omega;
 template <> struct Omega<float> { __host__ __device__ static constexpr float value() { return (float)(2.0 / 3.0); } };
 template <> struct Omega<double> { __host__ __device__ static constexpr double value() { return 2.0 / 3.0; } };
 
+// max of non-negative values that does NOT drop a NaN (fmax does): a NaN operand wins, so that a non-finite field shows
+// in the norm instead of reading as "converged".
+__device__ __forceinline__ double nanmax(double m, double a) { return (a != a || m != m) ? (m + a) : fmax(m, a); }
 // max over a warp / CTA of non-negative values, then one atomicMax on the bit pattern (exact, order-free:
-// the IEEE bit pattern of non-negative doubles is monotone in the value).
+// the IEEE bit pattern of non-negative doubles is monotone in the value, Inf and NaN above every finite one).
 __device__ __forceinline__ double warp_max(double v) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    for (int o = 16; o > 0; o >>= 1) v = nanmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     return v;
 }
 __device__ __forceinline__ double warp_sum(double v) {
@@ -77,7 +80,7 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
 }
 
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* slot, double v) {
-    atomicMax(slot, (unsigned long long)__double_as_longlong(v));
+    atomicMax(slot, (unsigned long long)__double_as_longlong(fabs(v)));   // fabs: a NaN with the sign bit set still sorts on top
 }
 
 // ---- solve bookkeeping of the lagged stop test, run by the LAST CTA of the level-0 launches -------------

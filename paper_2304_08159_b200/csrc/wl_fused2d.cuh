@@ -166,7 +166,7 @@ k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUte
                     const T c = (D[v] > (T)0) ? omega * ((T)1 / D[v]) : (T)0;
                     const T d = Ax[v] - bb[v];
                     if constexpr (RIN) {
-                        if (inside) rmax = fmax(rmax, fabs(d));
+                        if (inside) rmax = (d != d || rmax != rmax) ? (rmax + d) : fmax(rmax, fabs(d));
                     }
                     x1[v] = xc[v] + c * d;
                 }
@@ -221,7 +221,7 @@ k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUte
                 if constexpr (NORMS && !RIN) {
                     if (gx < P.N0 && gy < P.N1) {
 #pragma unroll
-                        for (int v = 0; v < VEC; ++v) rmax = fmax(rmax, fabs(r[v]));
+                        for (int v = 0; v < VEC; ++v) rmax = (r[v] != r[v] || rmax != rmax) ? (rmax + r[v]) : fmax(rmax, fabs(r[v]));
                     }
                 }
             }

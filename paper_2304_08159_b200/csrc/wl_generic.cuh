@@ -228,7 +228,7 @@ __global__ void k_absmax(long long M, const T* __restrict__ v, Scalars* scal, in
     __shared__ double red[32];
     double m = 0.0;
     for (long long I = (long long)blockIdx.x * blockDim.x + threadIdx.x; I < M; I += (long long)gridDim.x * blockDim.x)
-        m = fmax(m, fabs((double)v[I]));
+        m = nanmax(m, fabs((double)v[I]));
     m = block_max(m, red);
     if (threadIdx.x == 0) atomic_max_nonneg(&scal->absmax_bits[slot], m);
 }
@@ -244,7 +244,7 @@ __global__ void k_resnorm_sum(Grid g, const T* __restrict__ L, const T* __restri
         decompose<T, ND>(g, I, i0, i1, i2);
         T Ax, D;
         stencil_cell<T, ND>(g, L, p, I, i0, i1, i2, Ax, D);
-        m = fmax(m, fabs((double)(b[I] - Ax)));
+        m = nanmax(m, fabs((double)(b[I] - Ax)));
         s += (double)p[I];
     }
     m = block_max(m, red);

@@ -82,7 +82,7 @@ __global__ void k_pcg_residual(Grid g, const T* __restrict__ L, const T* __restr
         stencil_cell<T, ND>(g, L, x, I, i0, i1, i2, Ax, D);
         const T rv = b[I] - Ax;
         r[I] = rv;
-        m = fmax(m, fabs((double)rv));
+        m = nanmax(m, fabs((double)rv));
     }
     m = block_max(m, red);
     if (threadIdx.x == 0) atomic_max_nonneg(&scal->absmax_bits[1], m);
@@ -171,7 +171,7 @@ __global__ void k_pcg_update_xr(long long M, T* __restrict__ x, T* __restrict__ 
             const T aq = alpha * q[I];
             const T rv = r[I] - aq;
             r[I] = rv;
-            m = fmax(m, fabs((double)rv));
+            m = nanmax(m, fabs((double)rv));
         }
     }
     m = block_max(m, red);

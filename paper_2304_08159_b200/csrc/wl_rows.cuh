@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(kRowsX* kRowsY) k_divergence_rows(Grid g, cons
                 s += a1p[k] - a1[k];
                 if (ND == 3) s += a2p[k] - a2[k];
                 out[k] = s;
-                bmax = fmax(bmax, fabs(s));
+                bmax = (s != s || bmax != bmax) ? (bmax + s) : fmax(bmax, fabs(s));
             }
             st_vec<T, VEC>(b + r * g.N0 + x, out);
         }

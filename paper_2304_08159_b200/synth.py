@@ -259,6 +259,20 @@ def sphere_params(config: int, dims, count: int = 32, rmin: float = 8.0, rmax: f
     return centres, radii
 
 
+def body_records(kind: int, centres, radii, tube_radii=None) -> np.ndarray:
+    """The analytic bodies of a config as the 8-doubles-per-body records of ``wl_set_bodies`` (include/wl.h): kind (0 sphere
+    / circle, 1 torus about axis 0), c0, c1, c2, R, r, 0, 0.  A description of the INPUT geometry, no arithmetic."""
+    centres = np.asarray(centres, dtype=np.float64)
+    centres = centres.reshape(-1, centres.shape[-1])
+    rec = np.zeros((centres.shape[0], 8), dtype=np.float64)
+    rec[:, 0] = kind
+    rec[:, 1:1 + centres.shape[1]] = centres
+    rec[:, 4] = np.asarray(radii, dtype=np.float64).reshape(-1)
+    if tube_radii is not None:
+        rec[:, 5] = np.asarray(tube_radii, dtype=np.float64).reshape(-1)
+    return rec
+
+
 def make_config(config: int, dtype=None, scale: int = 1) -> dict:
     """Inputs of BASELINE.json ``configs[config]``; ``scale`` (a power of two) divides every grid
     extent and every body length by the same factor for reduced-size parity cases.
@@ -273,34 +287,39 @@ def make_config(config: int, dtype=None, scale: int = 1) -> dict:
     if config == 0:
         dims = (64 // s, 64 // s)
         L = coeff_uniform(dims, dt)
+        bodies = np.zeros((0, 8))
         u = velocity_uniform(dims, seed_for(0, 0), dt)
         tol, maxc, call = 0.0, 10, "solve"
     elif config == 1:
         dims = (1024 // s, 1024 // s)
         L = coeff_spheres(dims, [[256.0 / s, 512.0 / s]], [64.0 / s], dt)
+        bodies = body_records(0, [[256.0 / s, 512.0 / s]], [64.0 / s])
         u = velocity_uniform(dims, seed_for(1, 0), dt)
         tol, maxc, call = 1e-4, 32, "solve"
     elif config == 2:
         dims = (128 // s,) * 3
         L = coeff_spheres(dims, [[48.0 / s, 64.0 / s, 64.0 / s]], [24.0 / s], dt)
+        bodies = body_records(0, [[48.0 / s, 64.0 / s, 64.0 / s]], [24.0 / s])
         u = velocity_uniform(dims, seed_for(2, 0), dt)
         tol, maxc, call = 1e-4, 32, "project"
     elif config == 3:
         dims = (256 // s,) * 3
         L = coeff_uniform(dims, dt)
+        bodies = np.zeros((0, 8))
         u = velocity_taylor_green(dims, seed_for(3, 1), 1e-2, dt)
         tol, maxc, call = 1e-4, 32, "solve"
     elif config == 4:
         dims = (512 // s,) * 3
         centres, radii = sphere_params(4, dims, scale=s)
         L = coeff_spheres(dims, centres, radii, dt)
+        bodies = body_records(0, centres, radii)
         u = velocity_uniform(dims, seed_for(4, 0), dt)
         tol, maxc, call = 1e-4, 32, "project"
     else:
         raise ValueError(f"unknown config {config}")
     u *= L  # BDIM-masked velocity (stationary body); walls get u = 0
     return dict(config=config, name=CONFIG_NAMES[config] + (f"_div{s}" if s != 1 else ""),
-                dims=dims, dtype=dt, L=L, u=u, tol=tol, maxcycles=maxc, call=call)
+                dims=dims, dtype=dt, L=L, u=u, tol=tol, maxcycles=maxc, call=call, bodies=bodies)
 
 
 def make_donut(p: int, dtype=None) -> dict:
@@ -315,4 +334,4 @@ def make_donut(p: int, dtype=None) -> dict:
     u = velocity_uniform(dims, seed_for(5, int(p)), dt)
     u *= L
     return dict(config=5, name=f"donut_p{int(p)}_{dims[0]}x{dims[1]}x{dims[2]}", dims=dims, dtype=dt, L=L, u=u,
-                tol=1e-4, maxcycles=32, call="project")
+                tol=1e-4, maxcycles=32, call="project", bodies=body_records(1, [[n1, n1 / 2, n1 / 2]], [n1 / 4.0], [n1 / 16.0]))
