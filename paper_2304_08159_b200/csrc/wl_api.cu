@@ -33,7 +33,7 @@ constexpr int kTailSmemBudget = 200 * 1024;
 struct Level {
     Grid g;
     void* L = nullptr;      // n*M coefficients (ctx-owned copy / coarsened)
-    void* C = nullptr;      // M: omega / D per cell (0 where D = 0), derived from L by wl_set_coeff
+    void* C = nullptr;      // M: omega·(1/D) per cell (0 where D = 0), derived from L by wl_set_coeff; fp64 3-D contexts only
     void* x[2] = {nullptr, nullptr};  // level >= 1: iterate ping-pong; level 0: x[1] = ctx-owned scratch only
     void* b = nullptr;      // level >= 1: restricted residual
     void* tmp = nullptr;    // generic path only: second half of the Jacobi ping-pong (allocated on first use)
@@ -173,8 +173,9 @@ struct Impl {
             k_coarsen<T, ND><<<grid_for(c, b.g.M * ND), kBlock, 0, c->stream>>>(a.g, b.g, P(a.L), P(b.L));
             KCHECK(c, "k_coarsen");
         }
-        for (int l = 0; l < c->nlev; ++l) {   // omega / D per cell, once per coefficient set
+        for (int l = 0; USEC && ND == 3 && l < c->nlev; ++l) {   // omega·(1/D) per cell for the kernels that load it (fp64, 3-D)
             Level& v = c->lev[l];
+            if (!v.C) continue;
             if (rows_ok(v.g, v.L, v.C)) {
                 k_make_c_rows<T, ND><<<rows_grid(c, (long long)v.g.N1 * v.g.N2), dim3(kRowsX, kRowsY), 0, c->stream>>>(v.g, P(v.L), P(v.C));
                 KCHECK(c, "k_make_c_rows");
@@ -930,7 +931,7 @@ int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
     for (int l = 0; l < nlev; ++l) {
         Level& v = c->lev[l];
         dmalloc(&v.L, (size_t)v.g.M * ndim * c->esz);
-        dmalloc(&v.C, (size_t)v.g.M * c->esz);
+        if (dtype == WL_F64 && ndim == 3) dmalloc(&v.C, (size_t)v.g.M * c->esz);   // read by the fp64 fused kernels only
         dmalloc(&v.x[1], (size_t)v.g.M * c->esz);
         if (l > 0) {
             dmalloc(&v.x[0], (size_t)v.g.M * c->esz);
