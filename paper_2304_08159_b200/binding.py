@@ -48,6 +48,7 @@ SIGNATURES = {
     "wl_level_dims": (_i32, [_vp, _i32, _i64p]),
     "wl_get_coeff": (_i32, [_vp, _i32, _vp]),
     "wl_launch_count": (_i64, [_vp]),
+    "wl_plan_fused3d": (_i32, [_i64p, _i32, _i32, _i32, _i32p, _i32, _i32p, _i32p, _i64p]),
     "wl_last_error": (ctypes.c_char_p, [_vp]),
 }
 
@@ -252,6 +253,21 @@ def wl_get_coeff(ctx, level: int, out):
 
 def wl_launch_count(ctx) -> int:
     return int(load().wl_launch_count(ctx))
+
+
+def wl_plan_fused3d(dims, dtype, num_sms: int = 148):
+    """Work split of one fused 3-D level half (host only, no GPU): dims = (N_0, N_1, N_2) as in wl_create.
+    Returns (items[k] = (X0, Y0, z0, nz), start[grid + 1], load)."""
+    d = (ctypes.c_int64 * 3)(*[int(v) for v in dims])
+    dt = _dtype_code(dtype)
+    grid, load_ = ctypes.c_int(), ctypes.c_int64()
+    n = load().wl_plan_fused3d(d, dt, int(num_sms), 0, None, 0, None, ctypes.byref(grid), ctypes.byref(load_))
+    if n < 0:
+        raise WlError(n, "wl_plan_fused3d", "bad dims / dtype")
+    items = (ctypes.c_int * (4 * n))()
+    start = (ctypes.c_int * (grid.value + 1))()
+    load().wl_plan_fused3d(d, dt, int(num_sms), n, items, grid.value + 1, start, ctypes.byref(grid), ctypes.byref(load_))
+    return np.array(items, dtype=np.int64).reshape(n, 4), np.array(start, dtype=np.int64), int(load_.value)
 
 
 def wl_last_error(ctx) -> str:

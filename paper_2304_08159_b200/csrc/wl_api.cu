@@ -14,6 +14,7 @@
 #include "../../include/wl.h"
 #include "wl_common.cuh"
 #include "wl_generic.cuh"
+#include "wl_plan.h"
 #include "wl_fused3d.cuh"
 #include "wl_fused2d.cuh"
 #include "wl_tail.cuh"
@@ -37,6 +38,9 @@ struct Level {
     void* x[2] = {nullptr, nullptr};  // level >= 1: iterate ping-pong; level 0: x[1] = ctx-owned scratch only
     void* b = nullptr;      // level >= 1: restricted residual
     void* tmp = nullptr;    // generic path only: second half of the Jacobi ping-pong (allocated on first use)
+    int4* plan_items = nullptr;   // fused 3-D level half: per-CTA work lists (wl_plan.h), built on first use
+    int* plan_start = nullptr;
+    int plan_grid = 0;
 };
 
 thread_local char g_create_err[256] = "";
@@ -350,21 +354,9 @@ struct Impl {
             if (!ok) return fail(c, WL_ECUDA, "cuTensorMapEncodeTiled refused a level array (alignment?)");
             Fused3Params<T> prm;
             prm.N0 = f.g.N0; prm.N1 = f.g.N1; prm.N2 = f.g.N2;
-            prm.tiles_x = (f.g.N0 + FTX - 1) / FTX;
-            prm.tiles_y = (f.g.N1 + FTY - 1) / FTY;
-            // z-chunks: minimise waves * (planes per item + 6 run-in planes) over the chunk count (items dealt round-robin)
-            const long long ntiles = (long long)prm.tiles_x * prm.tiles_y;
-            const int half = f.g.N2 / 2;
-            long long best_cost = -1;
-            int best_nc = 1;
-            for (int nc = 1; nc <= half && nc <= 4096; ++nc) {
-                if (half / nc < 1 && nc > 1) break;                           // at least 2 planes per item
-                const long long items = ntiles * nc;
-                const long long waves = (items + c->num_sms - 1) / c->num_sms;
-                const long long cost = waves * (2LL * ((half + nc - 1) / nc) + 6);
-                if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_nc = nc; }
-            }
-            prm.nchunks = best_nc;
+            if (!f.plan_items) return fail(c, WL_ECUDA, "fused level without a work plan");
+            prm.items = f.plan_items;
+            prm.item_start = f.plan_start;
             prm.xout = P(x_out);
             prm.bc = P(bc);
             prm.scal = c->d_scal;
@@ -377,11 +369,9 @@ struct Impl {
             prm.check_done = c->check_done;
             auto kern = k_fused3d<T, FTX, FTY, FPF<PROLONG>, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN, USEC, TICKET>;
             constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF<PROLONG>, PROLONG, USEC>();
-            long long g = ntiles * best_nc;
-            if (g > c->num_sms) g = c->num_sms;
-            if (NORMS && g > kMaxPartials) g = kMaxPartials;
-            c->fused_grid = (int)g;
-            kern<<<(int)g, G::NT, smem, c->stream>>>(mx, mb, mL0, mL1, mL2, mC, mxc, prm);
+            const int g = f.plan_grid;
+            c->fused_grid = g;
+            kern<<<g, G::NT, smem, c->stream>>>(mx, mb, mL0, mL1, mL2, mC, mxc, prm);
             KCHECK(c, "k_fused3d");
             return WL_OK;
         } else {
@@ -577,6 +567,18 @@ struct Impl {
     // Set every opt-in shared-memory size once, outside any stream capture.
     static int init_kernels(wl_ctx* c) {
         if constexpr (ND == 3) {
+            // work plans of the fused level halves (every level that has a coarser one; tiny levels included: WL_OPT_FUSED = 2)
+            for (int l = 0; l + 1 < c->nlev; ++l) {
+                Level& v = c->lev[l];
+                const Plan pl = plan_fused3d(v.g.N0, v.g.N1, v.g.N2, FTX, FTY, c->num_sms);
+                static_assert(sizeof(PlanItem) == sizeof(int4), "plan items are uploaded as int4");
+                if (cudaMalloc((void**)&v.plan_items, pl.items.size() * sizeof(int4)) != cudaSuccess ||
+                    cudaMalloc((void**)&v.plan_start, pl.start.size() * sizeof(int)) != cudaSuccess)
+                    return fail(c, WL_ENOMEM, "cudaMalloc(work plan)");
+                CU(c, cudaMemcpy(v.plan_items, pl.items.data(), pl.items.size() * sizeof(int4), cudaMemcpyHostToDevice));
+                CU(c, cudaMemcpy(v.plan_start, pl.start.data(), pl.start.size() * sizeof(int), cudaMemcpyHostToDevice));
+                v.plan_grid = pl.grid();
+            }
             constexpr int s0 = (int)fused3d_smem_bytes<T, FTX, FTY, FPF<false>, false, USEC>(), s1 = (int)fused3d_smem_bytes<T, FTX, FTY, FPF<true>, true, USEC>();
             constexpr auto A = cudaFuncAttributeMaxDynamicSharedMemorySize;
             CU(c, cudaFuncSetAttribute(k_fused3d<T, FTX, FTY, FPF<false>, false, false, false, true, true, false, false, USEC, false>, A, s0));
@@ -986,6 +988,8 @@ void wl_destroy(wl_ctx* c) {
         if (v.x[1]) cudaFree(v.x[1]);
         if (v.b) cudaFree(v.b);
         if (v.tmp) cudaFree(v.tmp);
+        if (v.plan_items) cudaFree(v.plan_items);
+        if (v.plan_start) cudaFree(v.plan_start);
     }
     if (c->d_scal) cudaFree(c->d_scal);
     if (c->d_partials) cudaFree(c->d_partials);
@@ -1235,6 +1239,26 @@ int wl_get_coeff(const wl_ctx* c, int level, void* out) {
 }
 
 int64_t wl_launch_count(const wl_ctx* c) { return c ? c->launches : 0; }
+
+int wl_plan_fused3d(const int64_t* dims, int dtype, int num_sms, int cap_items, int* items_out, int cap_ctas, int* start_out,
+                    int* grid_out, int64_t* load_out) {
+    if (!dims || (dtype != WL_F32 && dtype != WL_F64) || num_sms < 1) return WL_EINVAL;
+    for (int i = 0; i < 3; ++i)
+        if (dims[i] < 2 || dims[i] > (1 << 20)) return WL_EDIMS;
+    if (dims[2] % 2) return WL_EDIMS;
+    const Plan pl = (dtype == WL_F32) ? plan_fused3d((int)dims[0], (int)dims[1], (int)dims[2], Impl<float, 3>::FTX, Impl<float, 3>::FTY, num_sms)
+                                      : plan_fused3d((int)dims[0], (int)dims[1], (int)dims[2], Impl<double, 3>::FTX, Impl<double, 3>::FTY, num_sms);
+    if (grid_out) *grid_out = pl.grid();
+    if (load_out) *load_out = pl.load;
+    if (items_out && start_out && (int)pl.items.size() <= cap_items && pl.grid() + 1 <= cap_ctas) {
+        for (size_t k = 0; k < pl.items.size(); ++k) {
+            items_out[4 * k] = pl.items[k].X0; items_out[4 * k + 1] = pl.items[k].Y0;
+            items_out[4 * k + 2] = pl.items[k].z0; items_out[4 * k + 3] = pl.items[k].nz;
+        }
+        for (size_t b = 0; b < pl.start.size(); ++b) start_out[b] = pl.start[b];
+    }
+    return (int)pl.items.size();
+}
 
 const char* wl_last_error(const wl_ctx* c) { return c ? c->err : g_create_err; }
 
