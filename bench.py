@@ -209,6 +209,7 @@ def main():
     ap.add_argument("--no-pcg", action="store_true", help="skip the conjugate-gradient leg (reported beside the V-cycle solver)")
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--graph", type=int, default=1)
+    ap.add_argument("--pdl", type=int, default=1, help="WL_OPT_PDL: programmatic dependent launch between the kernels of a cycle")
     ap.add_argument("--kernel-reps", type=int, default=20)
     args = ap.parse_args()
 
@@ -248,6 +249,7 @@ def main():
     pr = wl.Projector(dims, dt, dev)
     wl.wl_set_option(pr.ctx, wl.WL_OPT_FUSED, args.fused)
     wl.wl_set_option(pr.ctx, wl.WL_OPT_GRAPH, args.graph)
+    wl.wl_set_option(pr.ctx, wl.WL_OPT_PDL, args.pdl)
     u_host = torch.from_numpy(cfg["u"]).pin_memory()
     L_host = torch.from_numpy(cfg["L"]).pin_memory()
     u0 = u_host.to(dev, non_blocking=True)
@@ -394,7 +396,7 @@ def main():
         "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if dt == np.float32 else "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "dims": list(dims), "cells": M, "tol": tol, "maxcycles": maxc,
-                   "cycles_run": int(nc), "converged": bool(rc == 0), "fused": args.fused, "graph": args.graph,
+                   "cycles_run": int(nc), "converged": bool(rc == 0), "fused": args.fused, "graph": args.graph, "pdl": args.pdl,
                    "l2": "inputs larger than L2 (no flush needed)" if (n + 3) * M * esz > 200e6 else "working set fits L2",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "ms_per_projection": sec_per_step * 1e3,

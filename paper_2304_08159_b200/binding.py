@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libwl.so")
 WL_F32, WL_F64 = 0, 1
 WL_OK, WL_NOT_CONVERGED = 0, 1
 WL_EINVAL, WL_EDIMS, WL_ENOMEM, WL_ECUDA, WL_ESTATE, WL_ENONFINITE = -1, -2, -3, -4, -5, -6
-WL_OPT_FUSED, WL_OPT_GRAPH, WL_OPT_COARSE_CTA, WL_OPT_SOLVE_KERNELS, WL_OPT_SOLVER, WL_OPT_HOST_P_ZERO = 1, 2, 3, 4, 5, 6
+WL_OPT_FUSED, WL_OPT_GRAPH, WL_OPT_COARSE_CTA, WL_OPT_SOLVE_KERNELS, WL_OPT_SOLVER, WL_OPT_HOST_P_ZERO, WL_OPT_PDL = 1, 2, 3, 4, 5, 6, 7
 
 # every symbol include/wl.h declares: (restype, argtypes)
 _vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double

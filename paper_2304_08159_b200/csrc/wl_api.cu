@@ -9,6 +9,7 @@
 #include <initializer_list>
 #include <math.h>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "../../include/wl.h"
@@ -70,6 +71,8 @@ struct wl_ctx {
     int opt_host_p_zero = 0;     // WL_OPT_HOST_P_ZERO: wl_project_host starts from p = 0 without uploading p_host
     bool have_coeff = false;
     int opt_fused = 1, opt_graph = 1, opt_coarse_cta = 1, opt_solve_kernels = 0;
+    int opt_pdl = 1;             // WL_OPT_PDL: chain the cycle's kernels by programmatic dependent launch
+    bool pdl_armed = false;      // the last launch enqueued by the running call was a kernel that waits before touching data
     int num_sms = 148;
     // cached CUDA graph of one V-cycle (H9), valid for one (p, b, variant, stream, options) combination
     cudaStream_t own_stream = nullptr;   // the legacy default stream cannot be captured: graphs then run here, fenced by events
@@ -113,6 +116,31 @@ int fail(wl_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess) {
         cudaError_t e__ = cudaGetLastError();                            \
         if (e__ != cudaSuccess) return fail((c), WL_ECUDA, name, e__);   \
         (c)->launches++;                                                 \
+        (c)->pdl_armed = false;                                          \
+    } while (0)
+
+// Launch of a kernel that contains griddepcontrol.wait (fused level halves, coarse tail).  With WL_OPT_PDL it carries the
+// programmatic-serialization attribute when the launch before it (same API call, same stream) was such a kernel too, so that
+// the only things it reads before its wait — the level's coefficients and work plan — were written by an earlier, fully
+// ordered launch.  A stream capture turns the attribute into a programmatic edge of the graph.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_chained(wl_ctx* c, void (*kern)(KArgs...), int grid, int block, size_t smem, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = (c->opt_pdl && c->pdl_armed) ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+#define KCHAINED(c, name)                                                \
+    do {                                                                 \
+        KCHECK(c, name);                                                 \
+        (c)->pdl_armed = true;                                           \
     } while (0)
 
 inline int grid_for(const wl_ctx* c, long long work) {
@@ -325,9 +353,9 @@ struct Impl {
         prm.check_done = c->check_done;
         const int grid = prm.tiles_x * prm.tiles_y;
         c->fused_grid = grid;
-        k_fused2d<T, F2TX, F2TY, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN, TICKET>
-            <<<grid, G::NT, fused2d_smem_bytes<T, F2TX, F2TY>(), c->stream>>>(mx, mb, mL0, mL1, mxc, prm);
-        KCHECK(c, "k_fused2d");
+        launch_chained(c, k_fused2d<T, F2TX, F2TY, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN, TICKET>, grid, G::NT,
+                       fused2d_smem_bytes<T, F2TX, F2TY>(), mx, mb, mL0, mL1, mxc, prm);
+        KCHAINED(c, "k_fused2d");
         return WL_OK;
     }
 
@@ -371,8 +399,8 @@ struct Impl {
             constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF<PROLONG>, PROLONG, USEC>();
             const int g = f.plan_grid;
             c->fused_grid = g;
-            kern<<<g, G::NT, smem, c->stream>>>(mx, mb, mL0, mL1, mL2, mC, mxc, prm);
-            KCHECK(c, "k_fused3d");
+            launch_chained(c, kern, g, G::NT, smem, mx, mb, mL0, mL1, mL2, mC, mxc, prm);
+            KCHAINED(c, "k_fused3d");
             return WL_OK;
         } else {
             return launch_fused2<PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN, TICKET>(c, l, x_in, xc, b, x_out, bc);
@@ -416,8 +444,8 @@ struct Impl {
         prm.scal = c->d_scal;
         prm.check_done = c->check_done;
         auto kern = k_coarse_tail<T, ND>;
-        kern<<<1, kTailThreads, off, c->stream>>>(prm);
-        KCHECK(c, "k_coarse_tail");
+        launch_chained(c, kern, 1, kTailThreads, off, prm);
+        KCHAINED(c, "k_coarse_tail");
         return WL_OK;
     }
 
@@ -674,6 +702,7 @@ int run_cycle(wl_ctx* c, void* p, const void* b, bool in_solve, bool lagged, boo
     int rc;
     const int variant = pcg ? 4 : ((in_solve ? 1 : 0) | (lagged ? 2 : 0));
     auto enqueue = [&]() -> int {
+        c->pdl_armed = false;   // the first kernel of a cycle is fully ordered after whatever precedes it in the stream
         c->check_done = in_solve ? 1 : 0;
         int r = pcg ? DISPATCH(c, pcg_iteration)(c, p) : (lagged ? DISPATCH(c, cycle_lagged)(c, p, b) : DISPATCH(c, cycle)(c, p, b));
         c->check_done = 0;
@@ -1009,6 +1038,7 @@ void wl_destroy(wl_ctx* c) {
 int wl_set_stream(wl_ctx* c, void* s) {
     if (!c) return WL_EINVAL;
     if (c->stream != (cudaStream_t)s) drop_graph(c);
+    c->pdl_armed = false;
     c->stream = (cudaStream_t)s;
     return WL_OK;
 }
@@ -1023,6 +1053,7 @@ int wl_set_option(wl_ctx* c, int key, int value) {
         case WL_OPT_SOLVE_KERNELS: c->opt_solve_kernels = value ? 1 : 0; return WL_OK;
         case WL_OPT_SOLVER: c->opt_solver = value ? 1 : 0; return WL_OK;
         case WL_OPT_HOST_P_ZERO: c->opt_host_p_zero = value ? 1 : 0; return WL_OK;
+        case WL_OPT_PDL: c->opt_pdl = value ? 1 : 0; return WL_OK;
         default: return fail(c, WL_EINVAL, "wl_set_option: unknown key");
     }
 }
@@ -1187,6 +1218,7 @@ int wl_down(wl_ctx* c, int level, const void* x_in, const void* b, void* x_out, 
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_down: coefficients not set");
     if (c->opt_solve_kernels) { int rc = ensure_hist(c, 63); if (rc) return rc; }
     note_alignment(c, level, {x_in, b, x_out, bc});
+    c->pdl_armed = false;
     return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
 }
 
@@ -1196,6 +1228,7 @@ int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b,
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_up: coefficients not set");
     if (c->opt_solve_kernels) { int rc = ensure_hist(c, 63); if (rc) return rc; }
     note_alignment(c, level, {x_in, xc, b, x_out});
+    c->pdl_armed = false;
     return DISPATCH(c, up)(c, level, x_in, xc ? xc : c->lev[level + 1].x[1], b, x_out);
 }
 
@@ -1204,6 +1237,7 @@ int wl_vcycle_level(wl_ctx* c, int level, void* x, const void* b) {
     if (!x || !b) return fail(c, WL_EINVAL, "wl_vcycle_level: null pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_vcycle_level: coefficients not set");
     note_alignment(c, level, {x, b});
+    c->pdl_armed = false;
     return DISPATCH(c, vcycle)(c, level, x, b, level == 0 ? c->lev[0].x[1] : c->lev[level].x[0], x);
 }
 

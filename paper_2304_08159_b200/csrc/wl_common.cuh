@@ -33,6 +33,12 @@ struct Scalars {
     int pad;
 };
 
+// Programmatic dependent launch (sm_90+): `launch_dependents` lets the next kernel of the stream / graph start its prologue
+// while this grid is still running; `wait` blocks until every prerequisite grid has completed and its writes are visible.
+// Both are no-ops for a kernel launched without the programmatic-serialization attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 template <typename T> struct Omega;
 template <> struct Omega<float> { __host__ __device__ static constexpr float value() { return (float)(2.0 / 3.0); } };
 template <> struct Omega<double> { __host__ __device__ static constexpr double value() { return 2.0 / 3.0; } };

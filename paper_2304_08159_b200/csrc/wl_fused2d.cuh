@@ -89,7 +89,7 @@ k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUte
     constexpr uint32_t TX_BYTES = (uint32_t)((ZERO_IN ? 3 : 4) * G::PLANE * sizeof(T) + (PROLONG ? G::CWX * G::CWY * sizeof(T) : 0));
     static_assert(!RESTRICT || STAGE3, "restriction comes out of the residual stage");
     static_assert(!(RIN && ZERO_IN), "a zero input has residual b");
-    if (P.check_done && P.scal->done) return;
+    pdl_launch_dependents();   // the next kernel of the cycle may set up while this one runs (it waits before touching data)
 
     extern __shared__ __align__(1024) unsigned char smem2[];
     uint64_t* bar = (uint64_t*)smem2;
@@ -105,19 +105,31 @@ k_fused2d(const __grid_constant__ CUtensorMap tm_x, const __grid_constant__ CUte
     const T omega = Omega<T>::value();
 
     if (t == 0) {
-        mbar_init(bar, 1);
+        mbar_init(bar, 1);        // coefficients
+        mbar_init(bar + 1, 1);    // x, b, xc
         fence_mbar_init();
     }
     __syncthreads();
+    // The coefficients are written by no kernel of a cycle (and a kernel launched with the programmatic attribute always
+    // follows another kernel of the same cycle): their tiles are fetched while the predecessor is still draining.
     if (t == 0) {
-        mbar_expect_tx(bar, TX_BYTES);
-        if constexpr (!ZERO_IN) tma_load_2d(sx0, &tm_x, X0 - G::HX, Y0 - G::HY, bar);
-        tma_load_2d(sb, &tm_b, X0 - G::HX, Y0 - G::HY, bar);
+        mbar_expect_tx(bar, (uint32_t)(2 * G::PLANE * sizeof(T)));
         tma_load_2d(sl0, &tm_L0, X0 - G::HX, Y0 - G::HY, bar);
         tma_load_2d(sl1, &tm_L1, X0 - G::HX, Y0 - G::HY, bar);
-        if constexpr (PROLONG) tma_load_2d(sxc, &tm_xc, X0 / 2 - G::CH, Y0 / 2 - 2, bar);
+    }
+    pdl_wait();
+    if (P.check_done && P.scal->done) {   // uniform; no CTA may exit with a bulk copy into its shared memory in flight
+        mbar_wait(bar, 0);
+        return;
+    }
+    if (t == 0) {
+        mbar_expect_tx(bar + 1, TX_BYTES - (uint32_t)(2 * G::PLANE * sizeof(T)));
+        if constexpr (!ZERO_IN) tma_load_2d(sx0, &tm_x, X0 - G::HX, Y0 - G::HY, bar + 1);
+        tma_load_2d(sb, &tm_b, X0 - G::HX, Y0 - G::HY, bar + 1);
+        if constexpr (PROLONG) tma_load_2d(sxc, &tm_xc, X0 / 2 - G::CH, Y0 / 2 - 2, bar + 1);
     }
     mbar_wait(bar, 0);
+    mbar_wait(bar + 1, 0);
 
     // ---- stage 0: x0 += P xc, x0 -= mean (in place) -------------------------------------------------------------------
     if constexpr (!ZERO_IN && (PROLONG || SHIFT)) {

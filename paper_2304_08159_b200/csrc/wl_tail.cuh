@@ -141,7 +141,7 @@ __device__ __forceinline__ void tail_sweeps_cached(const Grid& g, const T* L, co
 
 template <typename T, int ND>
 __global__ void __launch_bounds__(kTailThreads, 1) k_coarse_tail(TailParams<T> P) {
-    if (P.check_done && P.scal->done) return;
+    pdl_launch_dependents();   // the next kernel of the cycle may set up while the tail runs (it waits before touching data)
     extern __shared__ __align__(16) unsigned char tail_smem[];
     auto XA = [&](int l) -> T* { return (T*)(tail_smem + P.off[l]); };
     auto XB = [&](int l) -> T* { return XA(l) + P.g[l].M; };
@@ -150,20 +150,12 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_coarse_tail(TailParams<T> P
     auto LL = [&](int l) -> T* { return XA(l) + 4 * P.g[l].M; };
     const T omega = Omega<T>::value();
 
-    // stage every level's coefficients, and the first level's b (and x) in shared memory
+    // Stage every level's coefficients in shared memory and derive omega/D from them.  No kernel of a cycle writes the
+    // coefficients, so under programmatic dependent launch this part runs while the level above is still draining.
     for (int l = 0; l < P.nl; ++l) {
         const int n = (int)P.g[l].M * ND;
         T* d = LL(l);
         for (int i = threadIdx.x; i < n; i += blockDim.x) d[i] = P.L[l][i];
-    }
-    {
-        const int M = (int)P.g[0].M;
-        T* b0 = B(0);
-        T* x0 = XA(0);
-        for (int i = threadIdx.x; i < M; i += blockDim.x) {
-            b0[i] = P.b_in[i];
-            if (!P.zero_in) x0[i] = P.x_in[i];
-        }
     }
     __syncthreads();
     for (int l = 0; l < P.nl; ++l) {   // C = omega * invD, D = sum of the cell's face coefficients (oracle order)
@@ -186,6 +178,17 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_coarse_tail(TailParams<T> P
             }
             const T invD = (D > (T)0) ? (T)1 / D : (T)0;
             C[I] = omega * invD;
+        }
+    }
+    pdl_wait();                                   // from here on: data the cycle's earlier kernels wrote
+    if (P.check_done && P.scal->done) return;     // uniform
+    {   // the first level's b (and x)
+        const int M = (int)P.g[0].M;
+        T* b0 = B(0);
+        T* x0 = XA(0);
+        for (int i = threadIdx.x; i < M; i += blockDim.x) {
+            b0[i] = P.b_in[i];
+            if (!P.zero_in) x0[i] = P.x_in[i];
         }
     }
     __syncthreads();
