@@ -53,6 +53,8 @@ def lib():
         L.orc_mu0.restype, L.orc_mu0.argtypes = f64, [f64]
         L.orc_body_coeff.restype, L.orc_body_coeff.argtypes = i32, [i32, i64p, i32, i32, f64p, vp]
         L.orc_solve_pcg.restype, L.orc_solve_pcg.argtypes = i32, [vp, vp, vp, f64, i32, f64p, i32p]
+        L.orc_convdiff.restype, L.orc_convdiff.argtypes = i32, [i32, i64p, i32, vp, f64, vp]
+        L.orc_face_value.restype, L.orc_face_value.argtypes = f64, [i32, f64, f64, f64]
         L.orc_divergence.restype, L.orc_divergence.argtypes = None, [vp, vp, vp]
         L.orc_gradient_correct.restype, L.orc_gradient_correct.argtypes = None, [vp, vp, vp]
         L.orc_remove_mean.restype, L.orc_remove_mean.argtypes = None, [vp, vp]
@@ -95,6 +97,25 @@ def body_coeff(dims, dtype, bodies) -> np.ndarray:
                               rec.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), _ptr(out))
     assert rc == 0
     return out
+
+
+def face_value(uu: float, c: float, d: float, dtype=np.float64) -> float:
+    """Limited third-order face value of (far-upstream, upstream, downstream) (NEXT-4)."""
+    return float(lib().orc_face_value(0 if np.dtype(dtype) == np.float32 else 1, float(uu), float(c), float(d)))
+
+
+def convdiff(u, nu: float) -> np.ndarray:
+    """r = convection + diffusion rate of change of the face field u, shape (n, N_{n-1}, ..., N_0) (NEXT-4)."""
+    u = np.ascontiguousarray(u)
+    assert u.dtype in (np.float32, np.float64)
+    n = u.shape[0]
+    dims = tuple(reversed(u.shape[1:]))
+    assert len(dims) == n
+    r = np.empty_like(u)
+    arr = (ctypes.c_int64 * n)(*dims)
+    rc = lib().orc_convdiff(n, arr, 0 if u.dtype == np.float32 else 1, _ptr(u), float(nu), _ptr(r))
+    assert rc == 0
+    return r
 
 
 class Oracle:

@@ -41,6 +41,16 @@
 //                  the cell-integral of 1 - L over a sphere reproduces its volume; face-centre
 //                  convention checked on a half-space-like huge sphere (tests/test_oracle_body.py).
 //
+//   convdiff       (`convdiff!`; "third-order finite volume")
+//                  pinned: the face value against Leonard's normalised-variable diagram written independently, exact
+//                  point value of any quadratic given by its cell averages, boundedness; the diffusive part
+//                  (r(nu=1) - r(nu=0)) against a Kronecker-sum Laplacian with free-slip walls; second-order
+//                  convergence to -(u.grad)u + nu lap u of the Taylor-Green field (signs, the 1/2 of the advecting
+//                  velocity, every index offset); a step profile advected both ways (upwind direction); mirror and
+//                  axis-permutation covariance; momentum conservation (tests/test_oracle_convdiff.py).  The scheme's
+//                  details are DESIGN.md section 3 reading 15: the paper prints none -> "parity unpinned" by any value
+//                  of the paper.
+//
 // Notation: n = ndim in {2,3}; N = (N_0..N_{n-1}), axis 0 unit-stride; cell I has
 // linear index I_0 + N_0 (I_1 + N_1 I_2); face (I,i) is the LOWER face of cell I in direction i
 // (coeff[I,i] multiplies p[I]-p[I-del(i)]).  L, u are n cell-sized fields back to
@@ -520,6 +530,90 @@ void body_coeff(const Dims& g, int nbodies, const double* bodies, T* L) {
                 }
 }
 
+// ---------------------------------------------------------------------------------------------
+// CONVDIFF (the paper's `convdiff!` routine; "a third-order finite
+// volume scheme ... implicit Large Eddy Simulation" PAPER.md:25).  The text gives the scheme's name only; every
+// detail below is DESIGN.md section 3 reading 15:
+//   r[i][I] = sum_j ( F_ij(I) - F_ij(I + d_j) )   for faces I_i >= 1,   r = 0 on the stored wall plane I_i = 0,
+//   F_ij(I) = flux of u_i in direction j through the lower-j face of the control volume of u[i][I]
+//           = U phi - nu (u[i][I] - u[i][I - d_j]),
+//   U   = (u[j][I] + u[j][I - d_i]) / 2                       (advecting velocity, linear interpolation to the flux point)
+//   phi = third-order upwind-biased face value of u_i along j: with C / D the values up / downstream of the flux point
+//         (U >= 0: C = u[i][I-d_j], D = u[i][I], UU = u[i][I-2d_j];  U < 0: C = u[i][I], D = u[i][I-d_j], UU = u[i][I+d_j])
+//         phi3 = (5 C + 2 D - UU) / 6   — the quadratic through three cell AVERAGES evaluated at the face (finite volume) —
+//         limited to the monotone range (Leonard's universal limiter, constant slope 10):
+//         phi = median(phi3, C, median(C, D, 10 C - 9 UU));  where UU lies outside the field, phi = (C + D) / 2.
+//   Closed, impermeable, free-slip box (the Neumann walls of the projection, BJ "zero on domain-boundary faces"):
+//   F_ij = 0 on the walls I_j = 0 and I_j = N_j for j != i; the unstored upper wall value u[i][N_i] is 0.
+// Values are "defined" for 0 <= K_a <= N_a - 1 on every axis a != i and 0 <= K_i <= N_i.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+T median3(T a, T b, T c) {
+    const T lo = (a < b) ? a : b;
+    const T hi = (a < b) ? b : a;
+    const T m = (hi < c) ? hi : c;
+    return (lo < m) ? m : lo;
+}
+
+template <class T>
+T face_value3(T uu, T c, T d) {
+    const T phi3 = (T(5) * c + T(2) * d - uu) / T(6);
+    const T bound = T(10) * c - T(9) * uu;
+    return median3(phi3, c, median3(c, d, bound));
+}
+
+template <class T>
+bool face_get(const Dims& g, const T* u, int i, const int64_t* K, T* v) {
+    for (int a = 0; a < g.n; ++a) {
+        if (K[a] < 0) return false;
+        if (K[a] > ((a == i) ? g.N[a] : g.N[a] - 1)) return false;
+    }
+    if (K[i] == g.N[i]) { *v = (T)0; return true; }
+    *v = u[(int64_t)i * g.M + K[0] + g.N[0] * (K[1] + g.N[1] * K[2])];
+    return true;
+}
+
+template <class T>
+T convdiff_flux(const Dims& g, const T* u, T nu, int i, int j, const int64_t* I) {
+    if (j != i && (I[j] == 0 || I[j] == g.N[j])) return (T)0;
+    int64_t K[3] = {I[0], I[1], I[2]};
+    T a = 0, b = 0, p0 = 0, m1 = 0, uu = 0;
+    face_get(g, u, j, K, &a);                 // u[j][I]
+    K[i] -= 1; face_get(g, u, j, K, &b);      // u[j][I - d_i]
+    K[i] += 1;
+    const T U = T(0.5) * (a + b);
+    face_get(g, u, i, K, &p0);                // u[i][I]
+    K[j] -= 1; face_get(g, u, i, K, &m1);     // u[i][I - d_j]
+    T C, D;
+    bool have;
+    if (U >= (T)0) { C = m1; D = p0; K[j] -= 1; have = face_get(g, u, i, K, &uu); }
+    else { C = p0; D = m1; K[j] += 2; have = face_get(g, u, i, K, &uu); }
+    const T phi = have ? face_value3(uu, C, D) : T(0.5) * (C + D);
+    return U * phi - nu * (p0 - m1);
+}
+
+template <class T>
+void convdiff(const Dims& g, const T* u, double nu_, T* r) {
+    const T nu = (T)nu_;
+    for (int i = 0; i < g.n; ++i)
+        for (int64_t I2 = 0; I2 < g.N[2]; ++I2)
+            for (int64_t I1 = 0; I1 < g.N[1]; ++I1)
+                for (int64_t I0 = 0; I0 < g.N[0]; ++I0) {
+                    const int64_t I[3] = {I0, I1, I2};
+                    T s = 0;
+                    if (I[i] > 0) {
+                        for (int j = 0; j < g.n; ++j) {
+                            int64_t Iu[3] = {I0, I1, I2};
+                            Iu[j] += 1;
+                            const T Fl = convdiff_flux(g, u, nu, i, j, I);
+                            const T Fu = convdiff_flux(g, u, nu, i, j, Iu);
+                            s = s + (Fl - Fu);
+                        }
+                    }
+                    r[(int64_t)i * g.M + I0 + g.N[0] * (I1 + g.N[1] * I2)] = s;
+                }
+}
+
 struct Handle {
     int dtype;  // 0 = f32, 1 = f64
     void* ctx;
@@ -676,6 +770,20 @@ void orc_gradient_correct(void* hv, void* u, const void* p) {
 void orc_remove_mean(void* hv, void* p) {
     Handle* h = (Handle*)hv;
     DISPATCH(h, remove_mean((T*)p, c->lev[0].g.M), remove_mean((T*)p, c->lev[0].g.M));
+}
+
+// NEXT-4: r = convdiff(u; nu) on a grid of `dims` (no context needed).  dtype 0 = f32, 1 = f64.
+int orc_convdiff(int ndim, const int64_t* dims, int dtype, const void* u, double nu, void* r) {
+    if (ndim < 2 || ndim > 3) return -1;
+    const Dims g = make_dims(ndim, dims);
+    if (dtype == 0) convdiff<float>(g, (const float*)u, nu, (float*)r);
+    else convdiff<double>(g, (const double*)u, nu, (double*)r);
+    return 0;
+}
+// the limited third-order face value of (UU, C, D), in the given precision (returned as double)
+double orc_face_value(int dtype, double uu, double c, double d) {
+    if (dtype == 0) return (double)face_value3<float>((float)uu, (float)c, (float)d);
+    return face_value3<double>(uu, c, d);
 }
 
 }  // extern "C"
