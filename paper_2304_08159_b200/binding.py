@@ -37,6 +37,7 @@ SIGNATURES = {
     "wl_project_host": (_i32, [_vp, _vp, _vp, _vp, _f64, _i32, _f64p, _i32p]),
     "wl_divergence": (_i32, [_vp, _vp, _vp]),
     "wl_gradient": (_i32, [_vp, _vp, _vp]),
+    "wl_convdiff": (_i32, [_vp, _vp, _f64, _vp]),
     "wl_jacobi": (_i32, [_vp, _i32, _vp, _vp, _i32]),
     "wl_residual_restrict": (_i32, [_vp, _i32, _vp, _vp, _vp]),
     "wl_prolong_correct": (_i32, [_vp, _i32, _vp, _vp]),
@@ -202,6 +203,10 @@ def wl_divergence(ctx, u, b):
 
 def wl_gradient(ctx, u, p):
     return _check(ctx, load().wl_gradient(ctx, _dptr(u), _dptr(p)), "wl_gradient")
+
+
+def wl_convdiff(ctx, u, nu: float, r):
+    return _check(ctx, load().wl_convdiff(ctx, _dptr(u), float(nu), _dptr(r)), "wl_convdiff")
 
 
 def wl_jacobi(ctx, level: int, x, b, sweeps: int):

@@ -22,6 +22,7 @@
 #include "wl_rows.cuh"
 #include "wl_pcg.cuh"
 #include "wl_body.cuh"
+#include "wl_convdiff.cuh"
 
 using namespace wl;
 
@@ -625,7 +626,63 @@ struct Impl {
             CU(c, cudaFuncSetAttribute(k_fused2d<T, F2TX, F2TY, true, false, false, false, false, true, false, true>, A, s2));
         }
         CU(c, cudaFuncSetAttribute(k_coarse_tail<T, ND>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTailSmemBudget));
+        if constexpr (ND == 3)
+            CU(c, cudaFuncSetAttribute(k_convdiff3d<T, CDTY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CD3<T, CDTY>::smem_bytes()));
         return WL_OK;
+    }
+
+    // NEXT-4: r = convdiff(u; nu).  Tiled TMA kernel for 3-D grids whose rows are whole 16-byte vectors, else one thread per cell.
+    static constexpr int CDTY = 8;
+    static int convdiff(wl_ctx* c, const void* u, double nu, void* r) {
+        const Grid& g = c->lev[0].g;
+        if constexpr (ND == 3) {
+            using G = CD3<T, CDTY>;
+            if (c->opt_fused != 0 && rows_ok(g, u, r)) {
+                CUtensorMap m[3];
+                const uint64_t d[3] = {(uint64_t)g.N0, (uint64_t)g.N1, (uint64_t)g.N2};
+                const uint32_t bx[3] = {(uint32_t)G::WX, (uint32_t)G::WY, 1u};
+                bool ok = true;
+                for (int i = 0; i < 3; ++i) ok = ok && encode_map(&m[i], P(u) + (long long)i * g.M, (int)sizeof(T), 3, d, bx);
+                if (!ok) return fail(c, WL_ECUDA, "cuTensorMapEncodeTiled refused the velocity field");
+                CdParams<T> prm;
+                prm.N0 = g.N0; prm.N1 = g.N1; prm.N2 = g.N2;
+                prm.ntx = (g.N0 + G::TX - 1) / G::TX;
+                prm.nty = (g.N1 + G::TY - 1) / G::TY;
+                prm.nz = convdiff_chunk(prm.ntx * prm.nty, g.N2, c->num_sms * convdiff_ctas_per_sm());
+                prm.nu = (T)nu;
+                prm.r = P(r);
+                prm.M = g.M;
+                const int nchunks = (g.N2 + prm.nz - 1) / prm.nz;
+                k_convdiff3d<T, CDTY><<<prm.ntx * prm.nty * nchunks, G::NT, G::smem_bytes(), c->stream>>>(m[0], m[1], m[2], prm);
+                KCHECK(c, "k_convdiff3d");
+                return WL_OK;
+            }
+        }
+        k_convdiff<T, ND><<<grid_for(c, g.M), kBlock, 0, c->stream>>>(g, P(u), (T)nu, P(r));
+        KCHECK(c, "k_convdiff");
+        return WL_OK;
+    }
+    static int convdiff_ctas_per_sm() {
+        const size_t b = CD3<T, CDTY>::smem_bytes() + 1024;
+        const int by_smem = (int)((size_t)227 * 1024 / b);
+        const int by_threads = 2048 / CD3<T, CDTY>::NT;
+        const int k = by_smem < by_threads ? by_smem : by_threads;
+        return k < 1 ? 1 : k;
+    }
+    // planes per z-chunk: the split of N2 that minimises waves x (planes + 1 extra flux step) over `slots` resident CTAs
+    static int convdiff_chunk(int tiles, int N2, int slots) {
+        int best = N2;
+        long long best_cost = -1;
+        for (int nch = 1; nch <= N2; ++nch) {
+            const int nz = (N2 + nch - 1) / nch;
+            const int real = (N2 + nz - 1) / nz;
+            const long long items = (long long)tiles * real;
+            const long long waves = (items + slots - 1) / slots;
+            const long long cost = waves * (nz + 2);
+            if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = nz; }
+            if (nz == 1) break;
+        }
+        return best;
     }
 
     // with_nb: also leave ||b||inf in slot 0 (fused into the row kernel; one more pass on the generic path)
@@ -1190,6 +1247,12 @@ int wl_gradient(wl_ctx* c, void* u, const void* p) {
     if (!u || !p) return fail(c, WL_EINVAL, "wl_gradient: null pointer");
     if (!c->have_coeff) return fail(c, WL_ESTATE, "wl_gradient: coefficients not set");
     return DISPATCH(c, gradient)(c, u, p);
+}
+
+int wl_convdiff(wl_ctx* c, const void* u, double nu, void* r) {
+    if (!c) return WL_EINVAL;
+    if (!u || !r || u == r) return fail(c, WL_EINVAL, "wl_convdiff: null or aliased pointer");
+    return DISPATCH(c, convdiff)(c, u, nu, r);
 }
 
 int wl_jacobi(wl_ctx* c, int level, void* x, const void* b, int sweeps) {

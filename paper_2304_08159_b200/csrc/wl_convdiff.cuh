@@ -1,0 +1,403 @@
+// wl_convdiff.cuh — NEXT-4: the convection + diffusion rate of change of the face velocity, the paper's
+// `convdiff!` routine ("a third-order finite volume scheme ... implicit Large Eddy Simulation",
+// PAPER.md:25).  The text names the scheme only; every detail is DESIGN.md §3 reading 15:
+//   r[i][I] = sum_j ( F_ij(I) - F_ij(I + d_j) )  on faces I_i >= 1,  r = 0 on the stored wall plane I_i = 0,
+//   F_ij(I) = U phi - nu (u[i][I] - u[i][I - d_j]),   U = (u[j][I] + u[j][I - d_i]) / 2,
+//   phi     = median(phi3, C, median(C, D, 10 C - 9 UU)),  phi3 = (5 C + 2 D - UU) / 6,  with C / D the values of u_i up /
+//             downstream of the flux point and UU the one beyond C (U >= 0: C = u[i][I-d_j], D = u[i][I], UU = u[i][I-2d_j];
+//             U < 0: C = u[i][I], D = u[i][I-d_j], UU = u[i][I+d_j]);  phi = (C + D) / 2 where UU lies outside the field;
+//   closed free-slip box: F_ij = 0 on the walls I_j = 0, N_j for j != i; the unstored upper wall value u[i][N_i] is 0.
+// Every operation rounds separately and in the order written (the library is compiled with -fmad=false); the medians are taken
+// with min / max, which pick the same VALUE as any comparison network (the sign of a zero may differ; NaN inputs are out of
+// contract), so for finite fields r equals the oracle's value for value.
+//
+// Two kernels: k_convdiff (any shape, 2-D / 3-D, one thread per cell, every flux evaluated by both cells it separates) and
+// k_convdiff3d (3-D, rows of whole 16-byte vectors): a CTA owns a 32·VEC x TY tile and marches along z; planes arrive by TMA
+// (zero fill beyond the box = the unstored upper wall values), a thread owns one 16-byte vector of one row and keeps its four-
+// plane z-window in registers, every flux is evaluated ONCE (x: 4+1 per thread, y: handed to the row below through shared
+// memory, z: carried to the next plane in registers).
+#pragma once
+#include <cuda.h>
+
+#include "wl_common.cuh"
+#include "wl_generic.cuh"
+#include "wl_tma.cuh"
+
+namespace wl {
+
+__device__ __forceinline__ float cd_min(float a, float b) { return fminf(a, b); }
+__device__ __forceinline__ float cd_max(float a, float b) { return fmaxf(a, b); }
+__device__ __forceinline__ double cd_min(double a, double b) { return fmin(a, b); }
+__device__ __forceinline__ double cd_max(double a, double b) { return fmax(a, b); }
+
+template <typename T>
+__device__ __forceinline__ T cd_med3(T a, T b, T c) {
+    return cd_max(cd_min(a, b), cd_min(cd_max(a, b), c));
+}
+
+// x / 6, correctly rounded.  fp32: q = RN(x·RN(1/6)), one exact remainder, one correction — equal to the IEEE quotient for
+// every finite x with |x| >= 2^-100 (checked exhaustively over all 2^32 bit patterns: tests/test_gpu_convdiff.py); smaller
+// magnitudes (and zeros, whose sign the correction would lose) take the division instruction sequence.
+__device__ __forceinline__ float cd_div6(float x) {
+    const float y = 0.16666667163372039794921875f;   // RN(1/6)
+    const float q = __fmul_rn(x, y);
+    const float r = fmaf(-6.0f, q, x);
+    const float q2 = fmaf(r, y, q);
+    if (!(fabsf(x) >= 7.888609052210118e-31f)) return x / 6.0f;   // 2^-100
+    return q2;
+}
+__device__ __forceinline__ double cd_div6(double x) { return x / 6.0; }
+
+// One face flux.  (a, b): the two values of the advecting component; m2, m1, p0, p1: the advected component at I-2d, I-d, I,
+// I+d along the flux direction; hm2 / hp1: whether I-2d / I+d lie inside the field.
+template <typename T>
+__device__ __forceinline__ T cd_flux(T a, T b, T m2, T m1, T p0, T p1, bool hm2, bool hp1, T nu) {
+    const T U = T(0.5) * (a + b);
+    const bool pos = U >= T(0);
+    const T C = pos ? m1 : p0;
+    const T D = pos ? p0 : m1;
+    const T UU = pos ? m2 : p1;
+    const bool have = pos ? hm2 : hp1;
+    const T phi3 = cd_div6(T(5) * C + T(2) * D - UU);
+    const T bound = T(10) * C - T(9) * UU;
+    const T lim = cd_med3(phi3, C, cd_med3(C, D, bound));
+    const T cen = T(0.5) * (C + D);
+    const T phi = have ? lim : cen;
+    return U * phi - nu * (p0 - m1);
+}
+
+// ---- any shape ------------------------------------------------------------------------------------------------------------
+// value of component c at K (K_c = N_c: the unstored upper wall, 0); caller guarantees 0 <= K_a <= N_a - 1 (a != c), 0 <= K_c <= N_c
+template <typename T, int ND>
+__device__ __forceinline__ T cd_at(const Grid& g, const T* __restrict__ u, int c, const int* K) {
+    const int N[3] = {g.N0, g.N1, g.N2};
+    if (K[c] == N[c]) return T(0);
+    return u[(long long)c * g.M + cell_index(g, K[0], K[1], ND == 3 ? K[2] : 0)];
+}
+
+// F_ij at I, straight from global memory.
+template <typename T, int ND>
+__device__ __forceinline__ T cd_flux_at(const Grid& g, const T* __restrict__ u, T nu, int i, int j, const int* I) {
+    const int N[3] = {g.N0, g.N1, g.N2};
+    if (j != i && (I[j] == 0 || I[j] == N[j])) return T(0);
+    int K[3] = {I[0], I[1], I[2]};
+    const T a = cd_at<T, ND>(g, u, j, K);
+    K[i] -= 1;
+    const T b = cd_at<T, ND>(g, u, j, K);
+    K[i] += 1;
+    const T p0 = cd_at<T, ND>(g, u, i, K);
+    K[j] -= 1;
+    const T m1 = cd_at<T, ND>(g, u, i, K);
+    const int top = (j == i) ? N[j] : N[j] - 1;   // last index of component i along j that holds a value
+    const bool hm2 = I[j] - 2 >= 0;
+    const bool hp1 = I[j] + 1 <= top;
+    T m2 = T(0), p1 = T(0);
+    if (hm2) { K[j] = I[j] - 2; m2 = cd_at<T, ND>(g, u, i, K); }
+    if (hp1) { K[j] = I[j] + 1; p1 = cd_at<T, ND>(g, u, i, K); }
+    return cd_flux<T>(a, b, m2, m1, p0, p1, hm2, hp1, nu);
+}
+
+template <typename T, int ND>
+__global__ void k_convdiff(Grid g, const T* __restrict__ u, T nu, T* __restrict__ r) {
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < g.M; e += (long long)gridDim.x * blockDim.x) {
+        int I[3];
+        decompose<T, ND>(g, e, I[0], I[1], I[2]);
+#pragma unroll
+        for (int i = 0; i < ND; ++i) {
+            T s = T(0);
+            if (I[i] > 0) {
+#pragma unroll
+                for (int j = 0; j < ND; ++j) {
+                    int Iu[3] = {I[0], I[1], I[2]};
+                    Iu[j] += 1;
+                    const T Fl = cd_flux_at<T, ND>(g, u, nu, i, j, I);
+                    const T Fu = cd_flux_at<T, ND>(g, u, nu, i, j, Iu);
+                    s = s + (Fl - Fu);
+                }
+            }
+            r[(long long)i * g.M + e] = s;
+        }
+    }
+}
+
+// ---- 3-D, tiled ------------------------------------------------------------------------------------------------------------
+template <typename T, int TY_>
+struct CD3 {
+    static constexpr int VEC = 16 / (int)sizeof(T);
+    static constexpr int TX = 32 * VEC;          // one warp = one row of the tile
+    static constexpr int TY = TY_;
+    static constexpr int WX = TX + 2 * VEC;      // box: VEC cells of halo on either side (the box starts on a 16-byte boundary)
+    static constexpr int WY = TY + 4;            // rows Y0-2 .. Y0+TY+1 (row Y0+TY is the flux-only row)
+    static constexpr int NW = TY + 1;            // warps: TY rows that own cells + one that only evaluates the y-fluxes of row TY
+    static constexpr int NT = 32 * NW;
+    static constexpr int NSLOT = 4;              // ring of planes: k (neighbours), k+1 (own values), two in flight
+    static constexpr int PLANE = (WX * WY + 31) / 32 * 32;   // elements of one component in a slot (TMA destinations: 128-byte aligned)
+    static constexpr int SLOT = 3 * PLANE;
+    static constexpr int FROW = TX;              // flux exchange: [2 buffers][3 components][NW rows][TX]
+    static constexpr int FBUF = 3 * NW * FROW;
+    static constexpr size_t smem_bytes() { return (size_t)(NSLOT * SLOT + 2 * FBUF) * sizeof(T) + 128 + NSLOT * 8; }
+};
+
+template <typename T>
+struct CdParams {
+    int N0, N1, N2;
+    int ntx, nty;      // tiles in x and y
+    int nz;            // planes per z-chunk
+    T nu;
+    T* r;
+    long long M;
+};
+
+template <typename T, int V> struct CdVec;
+template <> struct CdVec<float, 4> { typedef float4 type; };
+template <> struct CdVec<double, 2> { typedef double2 type; };
+
+template <typename T, int TY>
+__global__ void __launch_bounds__(CD3<T, TY>::NT, 1)
+k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUtensorMap m1, const __grid_constant__ CUtensorMap m2,
+             const CdParams<T> prm) {
+    using G = CD3<T, TY>;
+    constexpr int VEC = G::VEC;
+    typedef typename CdVec<T, VEC>::type V;
+
+    extern __shared__ unsigned char smem_raw[];
+    T* ring = reinterpret_cast<T*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+    T* fbuf = ring + G::NSLOT * G::SLOT;
+    uint64_t* full = reinterpret_cast<uint64_t*>(fbuf + 2 * G::FBUF);
+
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    // item: chunk-major, so that CTAs resident together sweep neighbouring tiles of one z-range (halo reuse in L2)
+    const int tiles = prm.ntx * prm.nty;
+    const int chunk = blockIdx.x / tiles;
+    const int tile = blockIdx.x - chunk * tiles;
+    const int ty = tile / prm.ntx, tx = tile - ty * prm.ntx;
+    const int X0 = tx * G::TX, Y0 = ty * G::TY;
+    const int z0 = chunk * prm.nz;
+    const int z1 = min(z0 + prm.nz, prm.N2);     // planes [z0, z1) are this item's
+    const int N0 = prm.N0, N1 = prm.N1, N2 = prm.N2;
+    const T nu = prm.nu;
+
+    if (t == 0) {
+#pragma unroll
+        for (int s = 0; s < G::NSLOT; ++s) mbar_init(&full[s], 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+
+    // plane q (z0-2 <= q <= z1+1) lives in slot (q - (z0-2)) mod NSLOT
+    auto issue = [&](int q) {
+        const int s = (q - (z0 - 2)) & (G::NSLOT - 1);
+        T* dst = ring + s * G::SLOT;
+        mbar_expect_tx(&full[s], (uint32_t)(3 * G::WX * G::WY * sizeof(T)));
+        tma_load_3d(dst, &m0, X0 - VEC, Y0 - 2, q, &full[s]);
+        tma_load_3d(dst + G::PLANE, &m1, X0 - VEC, Y0 - 2, q, &full[s]);
+        tma_load_3d(dst + 2 * G::PLANE, &m2, X0 - VEC, Y0 - 2, q, &full[s]);
+    };
+    if (t == 0) {
+#pragma unroll
+        for (int d = 0; d < G::NSLOT; ++d) issue(z0 - 2 + d);
+    }
+
+    const int yy = w + 2;                 // row of the box this thread's vector sits in
+    const int xx = VEC + lane * VEC;      // column
+    const int gx = X0 + lane * VEC, gy = Y0 + w;
+    const int own = yy * G::WX + xx;
+    const bool full_row = w < TY;         // owns cells (the last warp only evaluates y-fluxes)
+
+    // per-thread boundary predicates (x: per flux position e = 0..VEC; y: per row)
+    unsigned wallx = 0, hm2x = 0, hp1x0 = 0, hp1x = 0;   // bit e
+#pragma unroll
+    for (int e = 0; e <= VEC; ++e) {
+        const int X = gx + e;
+        if (X == 0 || X == N0) wallx |= 1u << e;
+        if (X - 2 >= 0) hm2x |= 1u << e;
+        if (X + 1 <= N0) hp1x0 |= 1u << e;       // component 0 holds a value at N0 (the wall, 0)
+        if (X + 1 <= N0 - 1) hp1x |= 1u << e;
+    }
+    const bool wally = (gy == 0 || gy == N1);
+    const bool hm2y = gy - 2 >= 0;
+    const bool hp1y1 = gy + 1 <= N1, hp1y = gy + 1 <= N1 - 1;
+
+    T win[3][4][VEC];     // z-window of the thread's own vector: planes k-2, k-1, k, k+1
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) win[c][0][e] = T(0);
+    T acc[3][VEC];        // plane k-1: 0 + (x-flux difference) + (y-flux difference), in that order
+    T fzp[3][VEC];        // lower z-flux of plane k-1
+    T u0r_prev = T(0);    // u0 at (gx+VEC, gy) on plane k-1 (advecting velocity of the extra x-flux of component 2)
+
+    auto ldv = [&](const T* p, T* out) {
+        const V v = *reinterpret_cast<const V*>(p);
+        if constexpr (VEC == 4) { out[0] = v.x; out[1] = v.y; out[2] = v.z; out[3] = v.w; }
+        else { out[0] = v.x; out[1] = v.y; }
+    };
+    auto ld2 = [&](const T* p, T* out) {   // two consecutive elements, 2·sizeof(T)-aligned
+        if constexpr (VEC == 4) { const float2 v = *reinterpret_cast<const float2*>(p); out[0] = v.x; out[1] = v.y; }
+        else { const double2 v = *reinterpret_cast<const double2*>(p); out[0] = v.x; out[1] = v.y; }
+    };
+
+    // prologue: planes z0-2, z0-1, z0 into the window
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        mbar_wait(&full[d], 0);
+        const T* s = ring + d * G::SLOT;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) ldv(s + c * G::PLANE + own, win[c][d + 1]);
+    }
+    {
+        const T* s = ring + 1 * G::SLOT;   // plane z0-1
+        u0r_prev = s[own + VEC];
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) { acc[c][e] = T(0); fzp[c][e] = T(0); }
+    __syncthreads();                       // slots 0 and 1 (planes z0-2, z0-1) are free
+    if (t == 0) {
+        if (z0 + 2 <= z1 + 1) issue(z0 + 2);
+        if (z0 + 3 <= z1 + 1) issue(z0 + 3);
+    }
+
+    for (int k = z0; k <= z1; ++k) {
+        // rotate the window and take the own values of plane k+1
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) { win[c][0][e] = win[c][1][e]; win[c][1][e] = win[c][2][e]; win[c][2][e] = win[c][3][e]; }
+        {
+            const int q = k + 1 - (z0 - 2);
+            const int s = q & (G::NSLOT - 1);
+            mbar_wait(&full[s], (uint32_t)((q / G::NSLOT) & 1));
+            const T* sp = ring + s * G::SLOT;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) ldv(sp + c * G::PLANE + own, win[c][3]);
+        }
+        const int sk = (k - (z0 - 2)) & (G::NSLOT - 1);
+        const T* pk = ring + sk * G::SLOT;              // plane k: in-plane neighbours
+        T* fb = fbuf + (k & 1) * G::FBUF;
+
+        const bool inplane = k < z1;                    // the step past the chunk only needs the z-fluxes
+        const bool wallz = (k == 0 || k == N2);
+        const bool hm2z = k - 2 >= 0;
+        const bool hp1z2 = k + 1 <= N2, hp1z = k + 1 <= N2 - 1;
+
+        T fx[3][VEC + 1];   // lower x-fluxes at gx .. gx+VEC
+        T fy[3][VEC];       // lower y-fluxes
+        T fz[3][VEC];       // lower z-fluxes
+        T u0r = T(0);
+
+        // x-extended rows of plane k: ext[c][0..VEC+3] = cells gx-2 .. gx+VEC+1
+        T ext[3][VEC + 4];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            ld2(pk + c * G::PLANE + own - 2, &ext[c][0]);
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) ext[c][2 + e] = win[c][2][e];
+            ld2(pk + c * G::PLANE + own + VEC, &ext[c][VEC + 2]);
+        }
+        u0r = ext[0][VEC + 2];
+
+        if (inplane) {
+            // rows gy-2, gy-1, gy+1 of plane k
+            T ym2[3][VEC], ym1[3][VEC], yp1[3][VEC];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                ldv(pk + c * G::PLANE + own - 2 * G::WX, ym2[c]);
+                ldv(pk + c * G::PLANE + own - G::WX, ym1[c]);
+                ldv(pk + c * G::PLANE + own + G::WX, yp1[c]);
+            }
+            // y-fluxes: advecting velocity u1 at I and at I - d_i
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) {
+                const T a = win[1][2][e];
+                T f0 = cd_flux<T>(a, ext[1][1 + e], ym2[0][e], ym1[0][e], win[0][2][e], yp1[0][e], hm2y, hp1y, nu);
+                T f1 = cd_flux<T>(a, ym1[1][e], ym2[1][e], ym1[1][e], win[1][2][e], yp1[1][e], hm2y, hp1y1, nu);
+                T f2 = cd_flux<T>(a, win[1][1][e], ym2[2][e], ym1[2][e], win[2][2][e], yp1[2][e], hm2y, hp1y, nu);
+                fy[0][e] = wally ? T(0) : f0;
+                fy[1][e] = f1;
+                fy[2][e] = wally ? T(0) : f2;
+            }
+            // hand the lower y-fluxes to the row below
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                V v;
+                if constexpr (VEC == 4) { v.x = fy[c][0]; v.y = fy[c][1]; v.z = fy[c][2]; v.w = fy[c][3]; }
+                else { v.x = fy[c][0]; v.y = fy[c][1]; }
+                *reinterpret_cast<V*>(fb + (c * G::NW + w) * G::FROW + lane * VEC) = v;
+            }
+            if (full_row) {
+                // x-fluxes at gx .. gx+VEC: advecting velocity u0 at I and at I - d_i
+                const T u0ym1_r = pk[own - G::WX + VEC];        // u0 at (gx+VEC, gy-1)
+#pragma unroll
+                for (int e = 0; e <= VEC; ++e) {
+                    const bool wl_ = (wallx >> e) & 1, h2 = (hm2x >> e) & 1, h10 = (hp1x0 >> e) & 1, h1 = (hp1x >> e) & 1;
+                    const T a = ext[0][2 + e];
+                    const T b1 = (e < VEC) ? ym1[0][e < VEC ? e : 0] : u0ym1_r;
+                    const T b2 = (e < VEC) ? win[0][1][e < VEC ? e : 0] : u0r_prev;
+                    T f0 = cd_flux<T>(a, ext[0][1 + e], ext[0][e], ext[0][1 + e], ext[0][2 + e], ext[0][3 + e], h2, h10, nu);
+                    T f1 = cd_flux<T>(a, b1, ext[1][e], ext[1][1 + e], ext[1][2 + e], ext[1][3 + e], h2, h1, nu);
+                    T f2 = cd_flux<T>(a, b2, ext[2][e], ext[2][1 + e], ext[2][2 + e], ext[2][3 + e], h2, h1, nu);
+                    fx[0][e] = f0;
+                    fx[1][e] = wl_ ? T(0) : f1;
+                    fx[2][e] = wl_ ? T(0) : f2;
+                }
+            }
+        }
+        if (full_row) {
+            // z-fluxes: advecting velocity u2 at I and at I - d_i
+            T ym1_2[VEC];
+            ldv(pk + 2 * G::PLANE + own - G::WX, ym1_2);
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) {
+                const T a = win[2][2][e];
+                T f0 = cd_flux<T>(a, ext[2][1 + e], win[0][0][e], win[0][1][e], win[0][2][e], win[0][3][e], hm2z, hp1z, nu);
+                T f1 = cd_flux<T>(a, ym1_2[e], win[1][0][e], win[1][1][e], win[1][2][e], win[1][3][e], hm2z, hp1z, nu);
+                T f2 = cd_flux<T>(a, win[2][1][e], win[2][0][e], win[2][1][e], win[2][2][e], win[2][3][e], hm2z, hp1z2, nu);
+                fz[0][e] = wallz ? T(0) : f0;
+                fz[1][e] = wallz ? T(0) : f1;
+                fz[2][e] = f2;
+            }
+        }
+        __syncthreads();   // y-fluxes of this plane are in fb; nobody reads slot sk any more
+        if (t == 0 && k + 4 <= z1 + 1) issue(k + 4);
+
+        if (full_row) {
+            // finish plane k-1: r = acc + (Fz(k-1) - Fz(k))
+            if (k > z0 && gx < N0 && gy < N1) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    T o[VEC];
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e) {
+                        o[e] = acc[c][e] + (fzp[c][e] - fz[c][e]);
+                        const bool wallface = (c == 0) ? (gx + e == 0) : (c == 1) ? (gy == 0) : (k - 1 == 0);
+                        if (wallface) o[e] = T(0);
+                    }
+                    V v;
+                    if constexpr (VEC == 4) { v.x = o[0]; v.y = o[1]; v.z = o[2]; v.w = o[3]; }
+                    else { v.x = o[0]; v.y = o[1]; }
+                    *reinterpret_cast<V*>(prm.r + (long long)c * prm.M + ((long long)gx + (long long)N0 * ((long long)gy + (long long)N1 * (k - 1)))) = v;
+                }
+            }
+            if (inplane) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    T fu[VEC];
+                    ldv(fb + (c * G::NW + w + 1) * G::FROW + lane * VEC, fu);
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e) {
+                        T s = T(0);
+                        s = s + (fx[c][e] - fx[c][e + 1]);
+                        s = s + (fy[c][e] - fu[e]);
+                        acc[c][e] = s;
+                        fzp[c][e] = fz[c][e];
+                    }
+                }
+            }
+        }
+        u0r_prev = u0r;
+    }
+}
+
+}  // namespace wl
