@@ -19,6 +19,8 @@
 #pragma once
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "wl_common.cuh"
 #include "wl_generic.cuh"
 #include "wl_tma.cuh"
@@ -35,30 +37,38 @@ __device__ __forceinline__ T cd_med3(T a, T b, T c) {
     return cd_max(cd_min(a, b), cd_min(cd_max(a, b), c));
 }
 
-// x / 6, correctly rounded.  fp32: q = RN(x·RN(1/6)), one exact remainder, one correction — equal to the IEEE quotient for
-// every finite x with |x| >= 2^-100 (checked exhaustively over all 2^32 bit patterns: tests/test_gpu_convdiff.py); smaller
-// magnitudes (and zeros, whose sign the correction would lose) take the division instruction sequence.
-__device__ __forceinline__ float cd_div6(float x) {
-    const float y = 0.16666667163372039794921875f;   // RN(1/6)
-    const float q = __fmul_rn(x, y);
-    const float r = fmaf(-6.0f, q, x);
-    const float q2 = fmaf(r, y, q);
-    if (!(fabsf(x) >= 7.888609052210118e-31f)) return x / 6.0f;   // 2^-100
-    return q2;
+// x / 6, correctly rounded.  fp32, fast form: q = RN(x·RN(1/6)), one exact remainder, one correction — equal to the IEEE
+// quotient for every finite x with |x| >= 2^-100 (all mantissas checked on the host: tests/test_div6.py) and for x = 0 up to
+// the sign of the zero.  Smaller non-zero magnitudes (a subnormal quotient) raise `tiny`, and the caller evaluates its group
+// of fluxes again with the division proper (EXACT): the hot path carries two integer instructions per flux instead of a
+// division sequence.
+template <bool EXACT>
+__device__ __forceinline__ float cd_div6(float x, bool& tiny) {
+    if constexpr (EXACT) {
+        return x / 6.0f;
+    } else {
+        const float y = 0.16666667163372039794921875f;   // RN(1/6)
+        const float q = __fmul_rn(x, y);
+        const float r = fmaf(-6.0f, q, x);
+        // 0 < |x| < 2^-100 on the bit pattern (the sign shifted out, zero wrapped to the top): one multiply-add, one compare
+        tiny = tiny || (__float_as_uint(x) * 2u - 2u < 2u * 0x0D800000u - 2u);
+        return fmaf(r, y, q);
+    }
 }
-__device__ __forceinline__ double cd_div6(double x) { return x / 6.0; }
+template <bool EXACT>
+__device__ __forceinline__ double cd_div6(double x, bool&) { return x / 6.0; }
 
 // One face flux.  (a, b): the two values of the advecting component; m2, m1, p0, p1: the advected component at I-2d, I-d, I,
 // I+d along the flux direction; hm2 / hp1: whether I-2d / I+d lie inside the field.
-template <typename T>
-__device__ __forceinline__ T cd_flux(T a, T b, T m2, T m1, T p0, T p1, bool hm2, bool hp1, T nu) {
+template <typename T, bool EXACT>
+__device__ __forceinline__ T cd_flux(T a, T b, T m2, T m1, T p0, T p1, bool hm2, bool hp1, T nu, bool& tiny) {
     const T U = T(0.5) * (a + b);
     const bool pos = U >= T(0);
     const T C = pos ? m1 : p0;
     const T D = pos ? p0 : m1;
     const T UU = pos ? m2 : p1;
     const bool have = pos ? hm2 : hp1;
-    const T phi3 = cd_div6(T(5) * C + T(2) * D - UU);
+    const T phi3 = cd_div6<EXACT>(T(5) * C + T(2) * D - UU, tiny);
     const T bound = T(10) * C - T(9) * UU;
     const T lim = cd_med3(phi3, C, cd_med3(C, D, bound));
     const T cen = T(0.5) * (C + D);
@@ -94,7 +104,8 @@ __device__ __forceinline__ T cd_flux_at(const Grid& g, const T* __restrict__ u, 
     T m2 = T(0), p1 = T(0);
     if (hm2) { K[j] = I[j] - 2; m2 = cd_at<T, ND>(g, u, i, K); }
     if (hp1) { K[j] = I[j] + 1; p1 = cd_at<T, ND>(g, u, i, K); }
-    return cd_flux<T>(a, b, m2, m1, p0, p1, hm2, hp1, nu);
+    bool tiny = false;
+    return cd_flux<T, true>(a, b, m2, m1, p0, p1, hm2, hp1, nu, tiny);
 }
 
 template <typename T, int ND>
@@ -135,7 +146,7 @@ struct CD3 {
     static constexpr int SLOT = 3 * PLANE;
     static constexpr int FROW = TX;              // flux exchange: [2 buffers][3 components][NW rows][TX]
     static constexpr int FBUF = 3 * NW * FROW;
-    static constexpr size_t smem_bytes() { return (size_t)(NSLOT * SLOT + 2 * FBUF) * sizeof(T) + 128 + NSLOT * 8; }
+    static constexpr size_t smem_bytes() { return (size_t)(NSLOT * SLOT + 2 * FBUF) * sizeof(T) + 128 + (NSLOT + 1) * 8; }
 };
 
 template <typename T>
@@ -164,6 +175,7 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     T* ring = reinterpret_cast<T*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
     T* fbuf = ring + G::NSLOT * G::SLOT;
     uint64_t* full = reinterpret_cast<uint64_t*>(fbuf + 2 * G::FBUF);
+    uint64_t* stepbar = full + G::NSLOT;
 
     const int t = threadIdx.x, lane = t & 31, w = t >> 5;
     // item: chunk-major, so that CTAs resident together sweep neighbouring tiles of one z-range (halo reuse in L2)
@@ -180,6 +192,7 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     if (t == 0) {
 #pragma unroll
         for (int s = 0; s < G::NSLOT; ++s) mbar_init(&full[s], 1);
+        mbar_init(stepbar, G::NW);
         fence_mbar_init();
     }
     __syncthreads();
@@ -203,6 +216,8 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     const int gx = X0 + lane * VEC, gy = Y0 + w;
     const int own = yy * G::WX + xx;
     const bool full_row = w < TY;         // owns cells (the last warp only evaluates y-fluxes)
+    const bool stores = full_row && gx < N0 && gy < N1;
+    const bool live_y = gx < N0 && gy <= N1;          // this thread's y-fluxes are used by somebody
 
     // per-thread boundary predicates (x: per flux position e = 0..VEC; y: per row)
     unsigned wallx = 0, hm2x = 0, hp1x0 = 0, hp1x = 0;   // bit e
@@ -219,10 +234,6 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     const bool hp1y1 = gy + 1 <= N1, hp1y = gy + 1 <= N1 - 1;
 
     T win[3][4][VEC];     // z-window of the thread's own vector: planes k-2, k-1, k, k+1
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int e = 0; e < VEC; ++e) win[c][0][e] = T(0);
     T acc[3][VEC];        // plane k-1: 0 + (x-flux difference) + (y-flux difference), in that order
     T fzp[3][VEC];        // lower z-flux of plane k-1
     T u0r_prev = T(0);    // u0 at (gx+VEC, gy) on plane k-1 (advecting velocity of the extra x-flux of component 2)
@@ -236,6 +247,12 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
         if constexpr (VEC == 4) { const float2 v = *reinterpret_cast<const float2*>(p); out[0] = v.x; out[1] = v.y; }
         else { const double2 v = *reinterpret_cast<const double2*>(p); out[0] = v.x; out[1] = v.y; }
     };
+    auto stv = [&](T* p, const T* in) {
+        V v;
+        if constexpr (VEC == 4) { v.x = in[0]; v.y = in[1]; v.z = in[2]; v.w = in[3]; }
+        else { v.x = in[0]; v.y = in[1]; }
+        *reinterpret_cast<V*>(p) = v;
+    };
 
     // prologue: planes z0-2, z0-1, z0 into the window
 #pragma unroll
@@ -245,33 +262,33 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
 #pragma unroll
         for (int c = 0; c < 3; ++c) ldv(s + c * G::PLANE + own, win[c][d + 1]);
     }
-    {
-        const T* s = ring + 1 * G::SLOT;   // plane z0-1
-        u0r_prev = s[own + VEC];
-    }
+    u0r_prev = (ring + 1 * G::SLOT)[own + VEC];   // plane z0-1
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int e = 0; e < VEC; ++e) { acc[c][e] = T(0); fzp[c][e] = T(0); }
+        for (int e = 0; e < VEC; ++e) { acc[c][e] = T(0); fzp[c][e] = T(0); win[c][0][e] = T(0); }
     __syncthreads();                       // slots 0 and 1 (planes z0-2, z0-1) are free
     if (t == 0) {
         if (z0 + 2 <= z1 + 1) issue(z0 + 2);
         if (z0 + 3 <= z1 + 1) issue(z0 + 3);
     }
 
+    // One plane step per iteration.  (Unrolling it four times to rotate the window by renaming was measured: the loop body no
+    // longer fits the instruction cache and the kernel runs 15 % slower; the 36 moves are cheaper.)
+    constexpr int Wm2 = 0, Wm1 = 1, W0 = 2, Wp1 = 3;
+#pragma unroll 1
     for (int k = z0; k <= z1; ++k) {
-        // rotate the window and take the own values of plane k+1
+        {   // own values of plane k+1
 #pragma unroll
-        for (int c = 0; c < 3; ++c)
+            for (int c = 0; c < 3; ++c)
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) { win[c][0][e] = win[c][1][e]; win[c][1][e] = win[c][2][e]; win[c][2][e] = win[c][3][e]; }
-        {
+                for (int e = 0; e < VEC; ++e) { win[c][0][e] = win[c][1][e]; win[c][1][e] = win[c][2][e]; win[c][2][e] = win[c][3][e]; }
             const int q = k + 1 - (z0 - 2);
             const int s = q & (G::NSLOT - 1);
             mbar_wait(&full[s], (uint32_t)((q / G::NSLOT) & 1));
             const T* sp = ring + s * G::SLOT;
 #pragma unroll
-            for (int c = 0; c < 3; ++c) ldv(sp + c * G::PLANE + own, win[c][3]);
+            for (int c = 0; c < 3; ++c) ldv(sp + c * G::PLANE + own, win[c][Wp1]);
         }
         const int sk = (k - (z0 - 2)) & (G::NSLOT - 1);
         const T* pk = ring + sk * G::SLOT;              // plane k: in-plane neighbours
@@ -282,117 +299,139 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
         const bool hm2z = k - 2 >= 0;
         const bool hp1z2 = k + 1 <= N2, hp1z = k + 1 <= N2 - 1;
 
-        T fx[3][VEC + 1];   // lower x-fluxes at gx .. gx+VEC
         T fy[3][VEC];       // lower y-fluxes
-        T fz[3][VEC];       // lower z-fluxes
         T u0r = T(0);
 
-        // x-extended rows of plane k: ext[c][0..VEC+3] = cells gx-2 .. gx+VEC+1
-        T ext[3][VEC + 4];
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            ld2(pk + c * G::PLANE + own - 2, &ext[c][0]);
-#pragma unroll
-            for (int e = 0; e < VEC; ++e) ext[c][2 + e] = win[c][2][e];
-            ld2(pk + c * G::PLANE + own + VEC, &ext[c][VEC + 2]);
-        }
-        u0r = ext[0][VEC + 2];
-
         if (inplane) {
-            // rows gy-2, gy-1, gy+1 of plane k
-            T ym2[3][VEC], ym1[3][VEC], yp1[3][VEC];
+            // y-fluxes: advecting velocity u1 at I and at I - d_i
+            T ym2[3][VEC], ym1[3][VEC], yp1[3][VEC];    // rows gy-2, gy-1, gy+1
+            T u1l[2];                                   // u1 at gx-2, gx-1
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 ldv(pk + c * G::PLANE + own - 2 * G::WX, ym2[c]);
                 ldv(pk + c * G::PLANE + own - G::WX, ym1[c]);
                 ldv(pk + c * G::PLANE + own + G::WX, yp1[c]);
             }
-            // y-fluxes: advecting velocity u1 at I and at I - d_i
+            ld2(pk + G::PLANE + own - 2, u1l);
+            auto yflux = [&](auto EX_) {
+                constexpr bool EX = decltype(EX_)::value;
+                bool tiny = false;
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) {
-                const T a = win[1][2][e];
-                T f0 = cd_flux<T>(a, ext[1][1 + e], ym2[0][e], ym1[0][e], win[0][2][e], yp1[0][e], hm2y, hp1y, nu);
-                T f1 = cd_flux<T>(a, ym1[1][e], ym2[1][e], ym1[1][e], win[1][2][e], yp1[1][e], hm2y, hp1y1, nu);
-                T f2 = cd_flux<T>(a, win[1][1][e], ym2[2][e], ym1[2][e], win[2][2][e], yp1[2][e], hm2y, hp1y, nu);
-                fy[0][e] = wally ? T(0) : f0;
-                fy[1][e] = f1;
-                fy[2][e] = wally ? T(0) : f2;
-            }
+                for (int e = 0; e < VEC; ++e) {
+                    const T a = win[1][W0][e];
+                    const T bl = (e == 0) ? u1l[1] : win[1][W0][e > 0 ? e - 1 : 0];
+                    const T f0 = cd_flux<T, EX>(a, bl, ym2[0][e], ym1[0][e], win[0][W0][e], yp1[0][e], hm2y, hp1y, nu, tiny);
+                    const T f1 = cd_flux<T, EX>(a, ym1[1][e], ym2[1][e], ym1[1][e], win[1][W0][e], yp1[1][e], hm2y, hp1y1, nu, tiny);
+                    const T f2 = cd_flux<T, EX>(a, win[1][Wm1][e], ym2[2][e], ym1[2][e], win[2][W0][e], yp1[2][e], hm2y, hp1y, nu, tiny);
+                    fy[0][e] = wally ? T(0) : f0;
+                    fy[1][e] = f1;
+                    fy[2][e] = wally ? T(0) : f2;
+                }
+                return tiny;
+            };
+            if (yflux(std::false_type{}) && live_y) yflux(std::true_type{});
             // hand the lower y-fluxes to the row below
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                V v;
-                if constexpr (VEC == 4) { v.x = fy[c][0]; v.y = fy[c][1]; v.z = fy[c][2]; v.w = fy[c][3]; }
-                else { v.x = fy[c][0]; v.y = fy[c][1]; }
-                *reinterpret_cast<V*>(fb + (c * G::NW + w) * G::FROW + lane * VEC) = v;
-            }
-            if (full_row) {
-                // x-fluxes at gx .. gx+VEC: advecting velocity u0 at I and at I - d_i
-                const T u0ym1_r = pk[own - G::WX + VEC];        // u0 at (gx+VEC, gy-1)
-#pragma unroll
-                for (int e = 0; e <= VEC; ++e) {
-                    const bool wl_ = (wallx >> e) & 1, h2 = (hm2x >> e) & 1, h10 = (hp1x0 >> e) & 1, h1 = (hp1x >> e) & 1;
-                    const T a = ext[0][2 + e];
-                    const T b1 = (e < VEC) ? ym1[0][e < VEC ? e : 0] : u0ym1_r;
-                    const T b2 = (e < VEC) ? win[0][1][e < VEC ? e : 0] : u0r_prev;
-                    T f0 = cd_flux<T>(a, ext[0][1 + e], ext[0][e], ext[0][1 + e], ext[0][2 + e], ext[0][3 + e], h2, h10, nu);
-                    T f1 = cd_flux<T>(a, b1, ext[1][e], ext[1][1 + e], ext[1][2 + e], ext[1][3 + e], h2, h1, nu);
-                    T f2 = cd_flux<T>(a, b2, ext[2][e], ext[2][1 + e], ext[2][2 + e], ext[2][3 + e], h2, h1, nu);
-                    fx[0][e] = f0;
-                    fx[1][e] = wl_ ? T(0) : f1;
-                    fx[2][e] = wl_ ? T(0) : f2;
-                }
-            }
+            for (int c = 0; c < 3; ++c) stv(fb + (c * G::NW + w) * G::FROW + lane * VEC, fy[c]);
         }
         if (full_row) {
-            // z-fluxes: advecting velocity u2 at I and at I - d_i
-            T ym1_2[VEC];
-            ldv(pk + 2 * G::PLANE + own - G::WX, ym1_2);
-#pragma unroll
-            for (int e = 0; e < VEC; ++e) {
-                const T a = win[2][2][e];
-                T f0 = cd_flux<T>(a, ext[2][1 + e], win[0][0][e], win[0][1][e], win[0][2][e], win[0][3][e], hm2z, hp1z, nu);
-                T f1 = cd_flux<T>(a, ym1_2[e], win[1][0][e], win[1][1][e], win[1][2][e], win[1][3][e], hm2z, hp1z, nu);
-                T f2 = cd_flux<T>(a, win[2][1][e], win[2][0][e], win[2][1][e], win[2][2][e], win[2][3][e], hm2z, hp1z2, nu);
-                fz[0][e] = wallz ? T(0) : f0;
-                fz[1][e] = wallz ? T(0) : f1;
-                fz[2][e] = f2;
-            }
-        }
-        __syncthreads();   // y-fluxes of this plane are in fb; nobody reads slot sk any more
-        if (t == 0 && k + 4 <= z1 + 1) issue(k + 4);
-
-        if (full_row) {
-            // finish plane k-1: r = acc + (Fz(k-1) - Fz(k))
-            if (k > z0 && gx < N0 && gy < N1) {
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    T o[VEC];
+            {
+                // z-fluxes: advecting velocity u2 at I and at I - d_i; then plane k-1 is complete: r = acc + (Fz(k-1) - Fz(k))
+                T fz[3][VEC];
+                T u2l[2], u2d[VEC];                     // u2 at gx-2, gx-1; u2 on row gy-1
+                ld2(pk + 2 * G::PLANE + own - 2, u2l);
+                ldv(pk + 2 * G::PLANE + own - G::WX, u2d);
+                auto zflux = [&](auto EX_) {
+                    constexpr bool EX = decltype(EX_)::value;
+                    bool tiny = false;
 #pragma unroll
                     for (int e = 0; e < VEC; ++e) {
-                        o[e] = acc[c][e] + (fzp[c][e] - fz[c][e]);
-                        const bool wallface = (c == 0) ? (gx + e == 0) : (c == 1) ? (gy == 0) : (k - 1 == 0);
-                        if (wallface) o[e] = T(0);
+                        const T a = win[2][W0][e];
+                        const T bl = (e == 0) ? u2l[1] : win[2][W0][e > 0 ? e - 1 : 0];
+                        const T f0 = cd_flux<T, EX>(a, bl, win[0][Wm2][e], win[0][Wm1][e], win[0][W0][e], win[0][Wp1][e], hm2z, hp1z, nu, tiny);
+                        const T f1 = cd_flux<T, EX>(a, u2d[e], win[1][Wm2][e], win[1][Wm1][e], win[1][W0][e], win[1][Wp1][e], hm2z, hp1z, nu, tiny);
+                        const T f2 = cd_flux<T, EX>(a, win[2][Wm1][e], win[2][Wm2][e], win[2][Wm1][e], win[2][W0][e], win[2][Wp1][e], hm2z, hp1z2, nu, tiny);
+                        fz[0][e] = wallz ? T(0) : f0;
+                        fz[1][e] = wallz ? T(0) : f1;
+                        fz[2][e] = f2;
                     }
-                    V v;
-                    if constexpr (VEC == 4) { v.x = o[0]; v.y = o[1]; v.z = o[2]; v.w = o[3]; }
-                    else { v.x = o[0]; v.y = o[1]; }
-                    *reinterpret_cast<V*>(prm.r + (long long)c * prm.M + ((long long)gx + (long long)N0 * ((long long)gy + (long long)N1 * (k - 1)))) = v;
+                    return tiny;
+                };
+                if (zflux(std::false_type{}) && stores) zflux(std::true_type{});
+                if (k > z0 && stores) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        T o[VEC];
+#pragma unroll
+                        for (int e = 0; e < VEC; ++e) {
+                            o[e] = acc[c][e] + (fzp[c][e] - fz[c][e]);
+                            const bool wallface = (c == 0) ? (gx + e == 0) : (c == 1) ? (gy == 0) : (k - 1 == 0);
+                            if (wallface) o[e] = T(0);
+                        }
+                        stv(prm.r + (long long)c * prm.M + ((long long)gx + (long long)N0 * ((long long)gy + (long long)N1 * (k - 1))), o);
+                    }
                 }
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e) fzp[c][e] = fz[c][e];
             }
             if (inplane) {
+                // x-fluxes at gx .. gx+VEC: advecting velocity u0 at I and at I - d_i.  These are the last reads of plane k.
+                T ext[3][VEC + 4];                      // x-extended rows: ext[c][0..VEC+3] = cells gx-2 .. gx+VEC+1
+                T u0d[VEC];                             // u0 on row gy-1
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    ld2(pk + c * G::PLANE + own - 2, &ext[c][0]);
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e) ext[c][2 + e] = win[c][W0][e];
+                    ld2(pk + c * G::PLANE + own + VEC, &ext[c][VEC + 2]);
+                }
+                ldv(pk + own - G::WX, u0d);
+                const T u0ym1_r = pk[own - G::WX + VEC];    // u0 at (gx+VEC, gy-1)
+                u0r = ext[0][VEC + 2];
+                __syncwarp();
+                if (lane == 0) mbar_arrive(stepbar);
+                auto xflux = [&](auto EX_) {
+                    constexpr bool EX = decltype(EX_)::value;
+                    bool tiny = false;
+                    T fx[3][VEC + 1];
+#pragma unroll
+                    for (int e = 0; e <= VEC; ++e) {
+                        const bool wl_ = (wallx >> e) & 1, h2 = (hm2x >> e) & 1, h10 = (hp1x0 >> e) & 1, h1 = (hp1x >> e) & 1;
+                        const T a = ext[0][2 + e];
+                        const T b1 = (e < VEC) ? u0d[e < VEC ? e : 0] : u0ym1_r;
+                        const T b2 = (e < VEC) ? win[0][Wm1][e < VEC ? e : 0] : u0r_prev;
+                        const T f0 = cd_flux<T, EX>(a, ext[0][1 + e], ext[0][e], ext[0][1 + e], ext[0][2 + e], ext[0][3 + e], h2, h10, nu, tiny);
+                        const T f1 = cd_flux<T, EX>(a, b1, ext[1][e], ext[1][1 + e], ext[1][2 + e], ext[1][3 + e], h2, h1, nu, tiny);
+                        const T f2 = cd_flux<T, EX>(a, b2, ext[2][e], ext[2][1 + e], ext[2][2 + e], ext[2][3 + e], h2, h1, nu, tiny);
+                        fx[0][e] = f0;
+                        fx[1][e] = wl_ ? T(0) : f1;
+                        fx[2][e] = wl_ ? T(0) : f2;
+                    }
+#pragma unroll
+                    for (int c = 0; c < 3; ++c)
+#pragma unroll
+                        for (int e = 0; e < VEC; ++e) acc[c][e] = T(0) + (fx[c][e] - fx[c][e + 1]);
+                    return tiny;
+                };
+                if (xflux(std::false_type{}) && stores) xflux(std::true_type{});
+            }
+        } else if (inplane) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(stepbar);
+        }
+        if (inplane) {
+            // everybody's y-fluxes of this plane are in fb, and nobody reads slot sk any more
+            mbar_wait(stepbar, (uint32_t)((k - z0) & 1));
+            if (t == 0 && k + 4 <= z1 + 1) issue(k + 4);
+            if (full_row) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     T fu[VEC];
                     ldv(fb + (c * G::NW + w + 1) * G::FROW + lane * VEC, fu);
 #pragma unroll
-                    for (int e = 0; e < VEC; ++e) {
-                        T s = T(0);
-                        s = s + (fx[c][e] - fx[c][e + 1]);
-                        s = s + (fy[c][e] - fu[e]);
-                        acc[c][e] = s;
-                        fzp[c][e] = fz[c][e];
-                    }
+                    for (int e = 0; e < VEC; ++e) acc[c][e] = acc[c][e] + (fy[c][e] - fu[e]);
                 }
             }
         }
