@@ -654,6 +654,7 @@ struct Impl {
                 prm.nu = (T)nu;
                 prm.r = P(r);
                 prm.M = g.M;
+                prm.negzero2 = 0x8000000080000000ULL;
                 const int nchunks = (g.N2 + prm.nz - 1) / prm.nz;
                 k_convdiff3d<T, CDTY><<<prm.ntx * prm.nty * nchunks, G::NT, G::smem_bytes(), c->stream>>>(m[0], m[1], m[2], prm);
                 KCHECK(c, "k_convdiff3d");

@@ -22,6 +22,7 @@
 #include <type_traits>
 
 #include "wl_common.cuh"
+#include "wl_fused3d.cuh"
 #include "wl_generic.cuh"
 #include "wl_tma.cuh"
 
@@ -58,22 +59,82 @@ __device__ __forceinline__ float cd_div6(float x, bool& tiny) {
 template <bool EXACT>
 __device__ __forceinline__ double cd_div6(double x, bool&) { return x / 6.0; }
 
+// Boundary flags travel as bit masks (all ones = true): `have ? a : b` is then one bitwise select, and a flag that is a
+// compile-time constant (the interior x-positions of a thread's vector) folds away.
+template <typename T> struct CdMask;
+template <> struct CdMask<float> { typedef unsigned int type; };
+template <> struct CdMask<double> { typedef unsigned long long type; };
+__device__ __forceinline__ float cd_bitsel(unsigned int m, float a, float b) {
+    return __uint_as_float((__float_as_uint(a) & m) | (__float_as_uint(b) & ~m));
+}
+__device__ __forceinline__ double cd_bitsel(unsigned long long m, double a, double b) {
+    return __longlong_as_double((long long)(((unsigned long long)__double_as_longlong(a) & m) | ((unsigned long long)__double_as_longlong(b) & ~m)));
+}
+
 // One face flux.  (a, b): the two values of the advecting component; m2, m1, p0, p1: the advected component at I-2d, I-d, I,
-// I+d along the flux direction; hm2 / hp1: whether I-2d / I+d lie inside the field.
+// I+d along the flux direction; hm2 / hp1: whether I-2d / I+d lie inside the field; wall: the face lies on an impermeable wall.
 template <typename T, bool EXACT>
-__device__ __forceinline__ T cd_flux(T a, T b, T m2, T m1, T p0, T p1, bool hm2, bool hp1, T nu, bool& tiny) {
+__device__ __forceinline__ T cd_flux(T a, T b, T m2, T m1, T p0, T p1, typename CdMask<T>::type hm2, typename CdMask<T>::type hp1,
+                                     typename CdMask<T>::type wall, T nu, bool& tiny) {
     const T U = T(0.5) * (a + b);
     const bool pos = U >= T(0);
     const T C = pos ? m1 : p0;
     const T D = pos ? p0 : m1;
     const T UU = pos ? m2 : p1;
-    const bool have = pos ? hm2 : hp1;
+    const typename CdMask<T>::type have = pos ? hm2 : hp1;
     const T phi3 = cd_div6<EXACT>(T(5) * C + T(2) * D - UU, tiny);
     const T bound = T(10) * C - T(9) * UU;
     const T lim = cd_med3(phi3, C, cd_med3(C, D, bound));
     const T cen = T(0.5) * (C + D);
-    const T phi = have ? lim : cen;
-    return U * phi - nu * (p0 - m1);
+    const T phi = cd_bitsel(have, lim, cen);
+    return cd_bitsel(wall, T(0), U * phi - nu * (p0 - m1));
+}
+
+// Two fluxes side by side (fp32): the additions and multiplications run as packed f32x2 instructions (two IEEE-rounded results
+// per issue slot; a product is fma(a, b, -0), see wl_fused3d.cuh), selects, medians and the tiny test stay per element.
+struct CdConst2 { u64 half, two, five, six_neg, nine, ten, y, nu, nz; };
+template <bool EXACT>
+__device__ __forceinline__ void cd_flux2(u64 a, u64 b, u64 m2, u64 m1, u64 p0, u64 p1, unsigned hm2, unsigned hp1, unsigned wall,
+                                         const CdConst2& k, bool& tiny, float& f0, float& f1) {
+    const u64 U = f2_mul(k.half, f2_add(a, b), k.nz);
+    float U0, U1, m20, m21, m10, m11, p00, p01, p10, p11;
+    f2_unpack(U, U0, U1);
+    f2_unpack(m2, m20, m21); f2_unpack(m1, m10, m11); f2_unpack(p0, p00, p01); f2_unpack(p1, p10, p11);
+    const bool pos0 = U0 >= 0.0f, pos1 = U1 >= 0.0f;
+    const float C0 = pos0 ? m10 : p00, C1 = pos1 ? m11 : p01;
+    const float D0 = pos0 ? p00 : m10, D1 = pos1 ? p01 : m11;
+    const float UU0 = pos0 ? m20 : p10, UU1 = pos1 ? m21 : p11;
+    const unsigned have0 = pos0 ? hm2 : hp1, have1 = pos1 ? hm2 : hp1;
+    const u64 C = f2_pack(C0, C1), D = f2_pack(D0, D1), UU = f2_pack(UU0, UU1);
+    const u64 x = f2_sub(f2_add(f2_mul(k.five, C, k.nz), f2_mul(k.two, D, k.nz)), UU);
+    float phi30, phi31;
+    if constexpr (EXACT) {
+        float x0, x1;
+        f2_unpack(x, x0, x1);
+        phi30 = x0 / 6.0f;
+        phi31 = x1 / 6.0f;
+    } else {
+        const u64 q = f2_mul(x, k.y, k.nz);
+        u64 r, q2;
+        asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(k.six_neg), "l"(q), "l"(x));
+        asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(q2) : "l"(r), "l"(k.y), "l"(q));
+        f2_unpack(q2, phi30, phi31);
+        tiny = tiny || ((unsigned)x * 2u - 2u < 2u * 0x0D800000u - 2u) || ((unsigned)(x >> 32) * 2u - 2u < 2u * 0x0D800000u - 2u);
+    }
+    const u64 bound = f2_sub(f2_mul(k.ten, C, k.nz), f2_mul(k.nine, UU, k.nz));
+    float b0, b1;
+    f2_unpack(bound, b0, b1);
+    const float lim0 = cd_med3(phi30, C0, cd_med3(C0, D0, b0));
+    const float lim1 = cd_med3(phi31, C1, cd_med3(C1, D1, b1));
+    const u64 cen = f2_mul(k.half, f2_add(C, D), k.nz);
+    float cen0, cen1;
+    f2_unpack(cen, cen0, cen1);
+    const u64 phi = f2_pack(cd_bitsel(have0, lim0, cen0), cd_bitsel(have1, lim1, cen1));
+    const u64 F = f2_sub(f2_mul(U, phi, k.nz), f2_mul(k.nu, f2_sub(p0, m1), k.nz));
+    float F0, F1;
+    f2_unpack(F, F0, F1);
+    f0 = cd_bitsel(wall, 0.0f, F0);
+    f1 = cd_bitsel(wall, 0.0f, F1);
 }
 
 // ---- any shape ------------------------------------------------------------------------------------------------------------
@@ -105,7 +166,8 @@ __device__ __forceinline__ T cd_flux_at(const Grid& g, const T* __restrict__ u, 
     if (hm2) { K[j] = I[j] - 2; m2 = cd_at<T, ND>(g, u, i, K); }
     if (hp1) { K[j] = I[j] + 1; p1 = cd_at<T, ND>(g, u, i, K); }
     bool tiny = false;
-    return cd_flux<T, true>(a, b, m2, m1, p0, p1, hm2, hp1, nu, tiny);
+    typedef typename CdMask<T>::type Mk;
+    return cd_flux<T, true>(a, b, m2, m1, p0, p1, hm2 ? ~Mk(0) : Mk(0), hp1 ? ~Mk(0) : Mk(0), Mk(0), nu, tiny);
 }
 
 template <typename T, int ND>
@@ -157,6 +219,7 @@ struct CdParams {
     T nu;
     T* r;
     long long M;
+    unsigned long long negzero2;   // two -0.0f: the addend that turns fma.rn.f32x2 into a product (wl_fused3d.cuh)
 };
 
 template <typename T, int V> struct CdVec;
@@ -171,8 +234,8 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     constexpr int VEC = G::VEC;
     typedef typename CdVec<T, VEC>::type V;
 
-    extern __shared__ unsigned char smem_raw[];
-    T* ring = reinterpret_cast<T*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    T* ring = reinterpret_cast<T*>(smem_raw);
     T* fbuf = ring + G::NSLOT * G::SLOT;
     uint64_t* full = reinterpret_cast<uint64_t*>(fbuf + 2 * G::FBUF);
     uint64_t* stepbar = full + G::NSLOT;
@@ -219,19 +282,22 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     const bool stores = full_row && gx < N0 && gy < N1;
     const bool live_y = gx < N0 && gy <= N1;          // this thread's y-fluxes are used by somebody
 
-    // per-thread boundary predicates (x: per flux position e = 0..VEC; y: per row)
-    unsigned wallx = 0, hm2x = 0, hp1x0 = 0, hp1x = 0;   // bit e
-#pragma unroll
-    for (int e = 0; e <= VEC; ++e) {
-        const int X = gx + e;
-        if (X == 0 || X == N0) wallx |= 1u << e;
-        if (X - 2 >= 0) hm2x |= 1u << e;
-        if (X + 1 <= N0) hp1x0 |= 1u << e;       // component 0 holds a value at N0 (the wall, 0)
-        if (X + 1 <= N0 - 1) hp1x |= 1u << e;
+    // per-thread boundary masks.  x: only the first two and the last two flux positions of a row can lie at a wall, so the
+    // masks of the other positions are compile-time constants.  y: one set per row.
+    typedef typename CdMask<T>::type Mk;
+    constexpr Mk kAll = ~Mk(0), kNone = Mk(0);
+    const Mk xl_in = (gx == 0) ? kNone : kAll;            // false where this vector starts at the lower x-wall
+    const Mk xr_in = (gx + VEC == N0) ? kNone : kAll;     // false where it ends at the upper x-wall
+    const Mk wally = (gy == 0 || gy == N1) ? kAll : kNone;
+    const Mk hm2y = (gy - 2 >= 0) ? kAll : kNone;
+    const Mk hp1y1 = (gy + 1 <= N1) ? kAll : kNone, hp1y = (gy + 1 <= N1 - 1) ? kAll : kNone;
+    CdConst2 k2;
+    if constexpr (VEC == 4) {
+        k2.half = f2_pack(0.5f, 0.5f); k2.two = f2_pack(2.0f, 2.0f); k2.five = f2_pack(5.0f, 5.0f); k2.six_neg = f2_pack(-6.0f, -6.0f);
+        k2.nine = f2_pack(9.0f, 9.0f); k2.ten = f2_pack(10.0f, 10.0f);
+        k2.y = f2_pack(0.16666667163372039794921875f, 0.16666667163372039794921875f);
+        k2.nu = f2_pack((float)prm.nu, (float)prm.nu); k2.nz = prm.negzero2;
     }
-    const bool wally = (gy == 0 || gy == N1);
-    const bool hm2y = gy - 2 >= 0;
-    const bool hp1y1 = gy + 1 <= N1, hp1y = gy + 1 <= N1 - 1;
 
     T win[3][4][VEC];     // z-window of the thread's own vector: planes k-2, k-1, k, k+1
     T acc[3][VEC];        // plane k-1: 0 + (x-flux difference) + (y-flux difference), in that order
@@ -295,9 +361,9 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
         T* fb = fbuf + (k & 1) * G::FBUF;
 
         const bool inplane = k < z1;                    // the step past the chunk only needs the z-fluxes
-        const bool wallz = (k == 0 || k == N2);
-        const bool hm2z = k - 2 >= 0;
-        const bool hp1z2 = k + 1 <= N2, hp1z = k + 1 <= N2 - 1;
+        const Mk wallz = (k == 0 || k == N2) ? kAll : kNone;
+        const Mk hm2z = (k - 2 >= 0) ? kAll : kNone;
+        const Mk hp1z2 = (k + 1 <= N2) ? kAll : kNone, hp1z = (k + 1 <= N2 - 1) ? kAll : kNone;
 
         T fy[3][VEC];       // lower y-fluxes
         T u0r = T(0);
@@ -316,16 +382,30 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
             auto yflux = [&](auto EX_) {
                 constexpr bool EX = decltype(EX_)::value;
                 bool tiny = false;
+                if constexpr (VEC == 4) {
 #pragma unroll
-                for (int e = 0; e < VEC; ++e) {
-                    const T a = win[1][W0][e];
-                    const T bl = (e == 0) ? u1l[1] : win[1][W0][e > 0 ? e - 1 : 0];
-                    const T f0 = cd_flux<T, EX>(a, bl, ym2[0][e], ym1[0][e], win[0][W0][e], yp1[0][e], hm2y, hp1y, nu, tiny);
-                    const T f1 = cd_flux<T, EX>(a, ym1[1][e], ym2[1][e], ym1[1][e], win[1][W0][e], yp1[1][e], hm2y, hp1y1, nu, tiny);
-                    const T f2 = cd_flux<T, EX>(a, win[1][Wm1][e], ym2[2][e], ym1[2][e], win[2][W0][e], yp1[2][e], hm2y, hp1y, nu, tiny);
-                    fy[0][e] = wally ? T(0) : f0;
-                    fy[1][e] = f1;
-                    fy[2][e] = wally ? T(0) : f2;
+                    for (int e = 0; e < VEC; e += 2) {
+                        const u64 a = f2_pack(win[1][W0][e], win[1][W0][e + 1]);
+                        const u64 bl = f2_pack((e == 0) ? u1l[1] : win[1][W0][e > 0 ? e - 1 : 0], win[1][W0][e]);
+                        cd_flux2<EX>(a, bl, f2_pack(ym2[0][e], ym2[0][e + 1]), f2_pack(ym1[0][e], ym1[0][e + 1]),
+                                     f2_pack(win[0][W0][e], win[0][W0][e + 1]), f2_pack(yp1[0][e], yp1[0][e + 1]), hm2y, hp1y, wally, k2, tiny,
+                                     fy[0][e], fy[0][e + 1]);
+                        cd_flux2<EX>(a, f2_pack(ym1[1][e], ym1[1][e + 1]), f2_pack(ym2[1][e], ym2[1][e + 1]), f2_pack(ym1[1][e], ym1[1][e + 1]),
+                                     f2_pack(win[1][W0][e], win[1][W0][e + 1]), f2_pack(yp1[1][e], yp1[1][e + 1]), hm2y, hp1y1, kNone, k2, tiny,
+                                     fy[1][e], fy[1][e + 1]);
+                        cd_flux2<EX>(a, f2_pack(win[1][Wm1][e], win[1][Wm1][e + 1]), f2_pack(ym2[2][e], ym2[2][e + 1]), f2_pack(ym1[2][e], ym1[2][e + 1]),
+                                     f2_pack(win[2][W0][e], win[2][W0][e + 1]), f2_pack(yp1[2][e], yp1[2][e + 1]), hm2y, hp1y, wally, k2, tiny,
+                                     fy[2][e], fy[2][e + 1]);
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e) {
+                        const T a = win[1][W0][e];
+                        const T bl = (e == 0) ? u1l[1] : win[1][W0][e > 0 ? e - 1 : 0];
+                        fy[0][e] = cd_flux<T, EX>(a, bl, ym2[0][e], ym1[0][e], win[0][W0][e], yp1[0][e], hm2y, hp1y, wally, nu, tiny);
+                        fy[1][e] = cd_flux<T, EX>(a, ym1[1][e], ym2[1][e], ym1[1][e], win[1][W0][e], yp1[1][e], hm2y, hp1y1, kNone, nu, tiny);
+                        fy[2][e] = cd_flux<T, EX>(a, win[1][Wm1][e], ym2[2][e], ym1[2][e], win[2][W0][e], yp1[2][e], hm2y, hp1y, wally, nu, tiny);
+                    }
                 }
                 return tiny;
             };
@@ -344,16 +424,30 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                 auto zflux = [&](auto EX_) {
                     constexpr bool EX = decltype(EX_)::value;
                     bool tiny = false;
+                    if constexpr (VEC == 4) {
 #pragma unroll
-                    for (int e = 0; e < VEC; ++e) {
-                        const T a = win[2][W0][e];
-                        const T bl = (e == 0) ? u2l[1] : win[2][W0][e > 0 ? e - 1 : 0];
-                        const T f0 = cd_flux<T, EX>(a, bl, win[0][Wm2][e], win[0][Wm1][e], win[0][W0][e], win[0][Wp1][e], hm2z, hp1z, nu, tiny);
-                        const T f1 = cd_flux<T, EX>(a, u2d[e], win[1][Wm2][e], win[1][Wm1][e], win[1][W0][e], win[1][Wp1][e], hm2z, hp1z, nu, tiny);
-                        const T f2 = cd_flux<T, EX>(a, win[2][Wm1][e], win[2][Wm2][e], win[2][Wm1][e], win[2][W0][e], win[2][Wp1][e], hm2z, hp1z2, nu, tiny);
-                        fz[0][e] = wallz ? T(0) : f0;
-                        fz[1][e] = wallz ? T(0) : f1;
-                        fz[2][e] = f2;
+                        for (int e = 0; e < VEC; e += 2) {
+                            const u64 a = f2_pack(win[2][W0][e], win[2][W0][e + 1]);
+                            const u64 bl = f2_pack((e == 0) ? u2l[1] : win[2][W0][e > 0 ? e - 1 : 0], win[2][W0][e]);
+                            cd_flux2<EX>(a, bl, f2_pack(win[0][Wm2][e], win[0][Wm2][e + 1]), f2_pack(win[0][Wm1][e], win[0][Wm1][e + 1]),
+                                         f2_pack(win[0][W0][e], win[0][W0][e + 1]), f2_pack(win[0][Wp1][e], win[0][Wp1][e + 1]), hm2z, hp1z, wallz, k2, tiny,
+                                         fz[0][e], fz[0][e + 1]);
+                            cd_flux2<EX>(a, f2_pack(u2d[e], u2d[e + 1]), f2_pack(win[1][Wm2][e], win[1][Wm2][e + 1]), f2_pack(win[1][Wm1][e], win[1][Wm1][e + 1]),
+                                         f2_pack(win[1][W0][e], win[1][W0][e + 1]), f2_pack(win[1][Wp1][e], win[1][Wp1][e + 1]), hm2z, hp1z, wallz, k2, tiny,
+                                         fz[1][e], fz[1][e + 1]);
+                            cd_flux2<EX>(a, f2_pack(win[2][Wm1][e], win[2][Wm1][e + 1]), f2_pack(win[2][Wm2][e], win[2][Wm2][e + 1]), f2_pack(win[2][Wm1][e], win[2][Wm1][e + 1]),
+                                         f2_pack(win[2][W0][e], win[2][W0][e + 1]), f2_pack(win[2][Wp1][e], win[2][Wp1][e + 1]), hm2z, hp1z2, kNone, k2, tiny,
+                                         fz[2][e], fz[2][e + 1]);
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < VEC; ++e) {
+                            const T a = win[2][W0][e];
+                            const T bl = (e == 0) ? u2l[1] : win[2][W0][e > 0 ? e - 1 : 0];
+                            fz[0][e] = cd_flux<T, EX>(a, bl, win[0][Wm2][e], win[0][Wm1][e], win[0][W0][e], win[0][Wp1][e], hm2z, hp1z, wallz, nu, tiny);
+                            fz[1][e] = cd_flux<T, EX>(a, u2d[e], win[1][Wm2][e], win[1][Wm1][e], win[1][W0][e], win[1][Wp1][e], hm2z, hp1z, wallz, nu, tiny);
+                            fz[2][e] = cd_flux<T, EX>(a, win[2][Wm1][e], win[2][Wm2][e], win[2][Wm1][e], win[2][W0][e], win[2][Wp1][e], hm2z, hp1z2, kNone, nu, tiny);
+                        }
                     }
                     return tiny;
                 };
@@ -398,16 +492,16 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                     T fx[3][VEC + 1];
 #pragma unroll
                     for (int e = 0; e <= VEC; ++e) {
-                        const bool wl_ = (wallx >> e) & 1, h2 = (hm2x >> e) & 1, h10 = (hp1x0 >> e) & 1, h1 = (hp1x >> e) & 1;
+                        const Mk h2 = (e < 2) ? xl_in : kAll;                         // gx+e-2 >= 0
+                        const Mk h10 = (e == VEC) ? xr_in : kAll;                     // gx+e+1 <= N0     (component 0 holds the wall value at N0)
+                        const Mk h1 = (e >= VEC - 1) ? xr_in : kAll;                  // gx+e+1 <= N0 - 1
+                        const Mk wl_ = (e == 0) ? ~xl_in : (e == VEC) ? ~xr_in : kNone;   // gx+e == 0 or N0
                         const T a = ext[0][2 + e];
                         const T b1 = (e < VEC) ? u0d[e < VEC ? e : 0] : u0ym1_r;
                         const T b2 = (e < VEC) ? win[0][Wm1][e < VEC ? e : 0] : u0r_prev;
-                        const T f0 = cd_flux<T, EX>(a, ext[0][1 + e], ext[0][e], ext[0][1 + e], ext[0][2 + e], ext[0][3 + e], h2, h10, nu, tiny);
-                        const T f1 = cd_flux<T, EX>(a, b1, ext[1][e], ext[1][1 + e], ext[1][2 + e], ext[1][3 + e], h2, h1, nu, tiny);
-                        const T f2 = cd_flux<T, EX>(a, b2, ext[2][e], ext[2][1 + e], ext[2][2 + e], ext[2][3 + e], h2, h1, nu, tiny);
-                        fx[0][e] = f0;
-                        fx[1][e] = wl_ ? T(0) : f1;
-                        fx[2][e] = wl_ ? T(0) : f2;
+                        fx[0][e] = cd_flux<T, EX>(a, ext[0][1 + e], ext[0][e], ext[0][1 + e], ext[0][2 + e], ext[0][3 + e], h2, h10, kNone, nu, tiny);
+                        fx[1][e] = cd_flux<T, EX>(a, b1, ext[1][e], ext[1][1 + e], ext[1][2 + e], ext[1][3 + e], h2, h1, wl_, nu, tiny);
+                        fx[2][e] = cd_flux<T, EX>(a, b2, ext[2][e], ext[2][1 + e], ext[2][2 + e], ext[2][3 + e], h2, h1, wl_, nu, tiny);
                     }
 #pragma unroll
                     for (int c = 0; c < 3; ++c)
