@@ -37,6 +37,23 @@ template <typename T>
 __device__ __forceinline__ T cd_med3(T a, T b, T c) {
     return cd_max(cd_min(a, b), cd_min(cd_max(a, b), c));
 }
+__device__ __forceinline__ float cd_min3(float a, float b, float c) {   // FMNMX3 (sm_100)
+    float r;
+    asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+    return r;
+}
+__device__ __forceinline__ double cd_min3(double a, double b, double c) { return fmin(fmin(a, b), c); }
+// +1 or -1 with the sign of d (d = D - C): multiplying the limiter's arguments by it mirrors a falling profile into a rising one.
+__device__ __forceinline__ float cd_sign1(float d) { return __uint_as_float((__float_as_uint(d) & 0x80000000u) | 0x3f800000u); }
+__device__ __forceinline__ double cd_sign1(double d) {
+    return __longlong_as_double((long long)(((unsigned long long)__double_as_longlong(d) & 0x8000000000000000ULL) | 0x3ff0000000000000ULL));
+}
+// median(phi3, C, median(C, D, bound)) for C <= D: the inner median is min(max(bound, C), D) >= C, so the outer one clamps
+// phi3 to [C, inner] — three instructions, the last a three-input minimum.  Same value as the comparison network.
+template <typename T>
+__device__ __forceinline__ T cd_limit_rising(T phi3, T C, T D, T bound) {
+    return cd_min3(cd_max(phi3, C), cd_max(bound, C), D);
+}
 
 // x / 6, correctly rounded.  fp32, fast form: q = RN(x·RN(1/6)), one exact remainder, one correction — equal to the IEEE
 // quotient for every finite x with |x| >= 2^-100 (all mantissas checked on the host: tests/test_div6.py) and for x = 0 up to
@@ -82,11 +99,14 @@ __device__ __forceinline__ T cd_flux(T a, T b, T m2, T m1, T p0, T p1, typename 
     const T D = pos ? p0 : m1;
     const T UU = pos ? m2 : p1;
     const typename CdMask<T>::type have = pos ? hm2 : hp1;
-    const T phi3 = cd_div6<EXACT>(T(5) * C + T(2) * D - UU, tiny);
-    const T bound = T(10) * C - T(9) * UU;
-    const T lim = cd_med3(phi3, C, cd_med3(C, D, bound));
-    const T cen = T(0.5) * (C + D);
-    const T phi = cd_bitsel(have, lim, cen);
+    // mirrored so that D' >= C' (negation commutes with every rounding below, so phi = sg * phi' exactly)
+    const T sg = cd_sign1(D - C);
+    const T Cm = sg * C, Dm = sg * D, UUm = sg * UU;
+    const T phi3 = cd_div6<EXACT>(T(5) * Cm + T(2) * Dm - UUm, tiny);
+    const T bound = T(10) * Cm - T(9) * UUm;
+    const T lim = cd_limit_rising(phi3, Cm, Dm, bound);
+    const T cen = T(0.5) * (Cm + Dm);
+    const T phi = sg * cd_bitsel(have, lim, cen);
     return cd_bitsel(wall, T(0), U * phi - nu * (p0 - m1));
 }
 
@@ -105,7 +125,11 @@ __device__ __forceinline__ void cd_flux2(u64 a, u64 b, u64 m2, u64 m1, u64 p0, u
     const float D0 = pos0 ? p00 : m10, D1 = pos1 ? p01 : m11;
     const float UU0 = pos0 ? m20 : p10, UU1 = pos1 ? m21 : p11;
     const unsigned have0 = pos0 ? hm2 : hp1, have1 = pos1 ? hm2 : hp1;
-    const u64 C = f2_pack(C0, C1), D = f2_pack(D0, D1), UU = f2_pack(UU0, UU1);
+    const u64 Cu = f2_pack(C0, C1), Du = f2_pack(D0, D1);
+    float d0, d1;
+    f2_unpack(f2_sub(Du, Cu), d0, d1);
+    const u64 sg = f2_pack(cd_sign1(d0), cd_sign1(d1));   // mirror each flux so that D >= C (see cd_flux)
+    const u64 C = f2_mul(sg, Cu, k.nz), D = f2_mul(sg, Du, k.nz), UU = f2_mul(sg, f2_pack(UU0, UU1), k.nz);
     const u64 x = f2_sub(f2_add(f2_mul(k.five, C, k.nz), f2_mul(k.two, D, k.nz)), UU);
     float phi30, phi31;
     if constexpr (EXACT) {
@@ -122,14 +146,16 @@ __device__ __forceinline__ void cd_flux2(u64 a, u64 b, u64 m2, u64 m1, u64 p0, u
         tiny = tiny || ((unsigned)x * 2u - 2u < 2u * 0x0D800000u - 2u) || ((unsigned)(x >> 32) * 2u - 2u < 2u * 0x0D800000u - 2u);
     }
     const u64 bound = f2_sub(f2_mul(k.ten, C, k.nz), f2_mul(k.nine, UU, k.nz));
-    float b0, b1;
+    float b0, b1, Cm0, Cm1, Dm0, Dm1;
     f2_unpack(bound, b0, b1);
-    const float lim0 = cd_med3(phi30, C0, cd_med3(C0, D0, b0));
-    const float lim1 = cd_med3(phi31, C1, cd_med3(C1, D1, b1));
+    f2_unpack(C, Cm0, Cm1);
+    f2_unpack(D, Dm0, Dm1);
+    const float lim0 = cd_limit_rising(phi30, Cm0, Dm0, b0);
+    const float lim1 = cd_limit_rising(phi31, Cm1, Dm1, b1);
     const u64 cen = f2_mul(k.half, f2_add(C, D), k.nz);
     float cen0, cen1;
     f2_unpack(cen, cen0, cen1);
-    const u64 phi = f2_pack(cd_bitsel(have0, lim0, cen0), cd_bitsel(have1, lim1, cen1));
+    const u64 phi = f2_mul(sg, f2_pack(cd_bitsel(have0, lim0, cen0), cd_bitsel(have1, lim1, cen1)), k.nz);
     const u64 F = f2_sub(f2_mul(U, phi, k.nz), f2_mul(k.nu, f2_sub(p0, m1), k.nz));
     float F0, F1;
     f2_unpack(F, F0, F1);
@@ -203,7 +229,7 @@ struct CD3 {
     static constexpr int WY = TY + 4;            // rows Y0-2 .. Y0+TY+1 (row Y0+TY is the flux-only row)
     static constexpr int NW = TY + 1;            // warps: TY rows that own cells + one that only evaluates the y-fluxes of row TY
     static constexpr int NT = 32 * NW;
-    static constexpr int NSLOT = 4;              // ring of planes: k (neighbours), k+1 (own values), two in flight
+    static constexpr int NSLOT = 6;              // ring of planes: k-2 .. k+1 (the z-window is read from here), two in flight
     static constexpr int PLANE = (WX * WY + 31) / 32 * 32;   // elements of one component in a slot (TMA destinations: 128-byte aligned)
     static constexpr int SLOT = 3 * PLANE;
     static constexpr int FROW = TX;              // flux exchange: [2 buffers][3 components][NW rows][TX]
@@ -261,8 +287,9 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     __syncthreads();
 
     // plane q (z0-2 <= q <= z1+1) lives in slot (q - (z0-2)) mod NSLOT
+    const int qlast = z1 + 1;
     auto issue = [&](int q) {
-        const int s = (q - (z0 - 2)) & (G::NSLOT - 1);
+        const int s = (q - (z0 - 2)) % G::NSLOT;
         T* dst = ring + s * G::SLOT;
         mbar_expect_tx(&full[s], (uint32_t)(3 * G::WX * G::WY * sizeof(T)));
         tma_load_3d(dst, &m0, X0 - VEC, Y0 - 2, q, &full[s]);
@@ -271,7 +298,8 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     };
     if (t == 0) {
 #pragma unroll
-        for (int d = 0; d < G::NSLOT; ++d) issue(z0 - 2 + d);
+        for (int d = 0; d < G::NSLOT; ++d)
+            if (z0 - 2 + d <= qlast) issue(z0 - 2 + d);
     }
 
     const int yy = w + 2;                 // row of the box this thread's vector sits in
@@ -299,11 +327,8 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
         k2.nu = f2_pack((float)prm.nu, (float)prm.nu); k2.nz = prm.negzero2;
     }
 
-    T win[3][4][VEC];     // z-window of the thread's own vector: planes k-2, k-1, k, k+1
     T acc[3][VEC];        // plane k-1: 0 + (x-flux difference) + (y-flux difference), in that order
     T fzp[3][VEC];        // lower z-flux of plane k-1
-    T u0r_prev = T(0);    // u0 at (gx+VEC, gy) on plane k-1 (advecting velocity of the extra x-flux of component 2)
-
     auto ldv = [&](const T* p, T* out) {
         const V v = *reinterpret_cast<const V*>(p);
         if constexpr (VEC == 4) { out[0] = v.x; out[1] = v.y; out[2] = v.z; out[3] = v.w; }
@@ -320,44 +345,32 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
         *reinterpret_cast<V*>(p) = v;
     };
 
-    // prologue: planes z0-2, z0-1, z0 into the window
+    // prologue: planes z0-2, z0-1, z0 have landed
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        mbar_wait(&full[d], 0);
-        const T* s = ring + d * G::SLOT;
-#pragma unroll
-        for (int c = 0; c < 3; ++c) ldv(s + c * G::PLANE + own, win[c][d + 1]);
-    }
-    u0r_prev = (ring + 1 * G::SLOT)[own + VEC];   // plane z0-1
+    for (int d = 0; d < 3; ++d) mbar_wait(&full[d], 0);
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int e = 0; e < VEC; ++e) { acc[c][e] = T(0); fzp[c][e] = T(0); win[c][0][e] = T(0); }
-    __syncthreads();                       // slots 0 and 1 (planes z0-2, z0-1) are free
-    if (t == 0) {
-        if (z0 + 2 <= z1 + 1) issue(z0 + 2);
-        if (z0 + 3 <= z1 + 1) issue(z0 + 3);
-    }
+        for (int e = 0; e < VEC; ++e) { acc[c][e] = T(0); fzp[c][e] = T(0); }
 
-    // One plane step per iteration.  (Unrolling it four times to rotate the window by renaming was measured: the loop body no
-    // longer fits the instruction cache and the kernel runs 15 % slower; the 36 moves are cheaper.)
+    // One plane step per iteration.  The thread's z-window (its own vector on planes k-2 .. k+1) is read from the ring where it
+    // is needed instead of being carried in registers (36 registers and as many moves per step less; carrying it was measured:
+    // spills under the 168-register cap of 12 warps).
     constexpr int Wm2 = 0, Wm1 = 1, W0 = 2, Wp1 = 3;
+    int s0 = 2, sp1 = 3;            // slots of planes k and k+1
+    uint32_t php1 = 0;              // phase of plane k+1's slot
 #pragma unroll 1
     for (int k = z0; k <= z1; ++k) {
-        {   // own values of plane k+1
+        mbar_wait(&full[sp1], php1);
+        const int sm1 = (s0 == 0) ? G::NSLOT - 1 : s0 - 1;
+        const int sm2 = (sm1 == 0) ? G::NSLOT - 1 : sm1 - 1;
+        const T* pk = ring + s0 * G::SLOT;              // plane k: own values and in-plane neighbours
+        const T* pkm1 = ring + sm1 * G::SLOT;
+        const T* pkm2 = ring + sm2 * G::SLOT;
+        const T* pkp1 = ring + sp1 * G::SLOT;
+        T win[3][4][VEC];
 #pragma unroll
-            for (int c = 0; c < 3; ++c)
-#pragma unroll
-                for (int e = 0; e < VEC; ++e) { win[c][0][e] = win[c][1][e]; win[c][1][e] = win[c][2][e]; win[c][2][e] = win[c][3][e]; }
-            const int q = k + 1 - (z0 - 2);
-            const int s = q & (G::NSLOT - 1);
-            mbar_wait(&full[s], (uint32_t)((q / G::NSLOT) & 1));
-            const T* sp = ring + s * G::SLOT;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) ldv(sp + c * G::PLANE + own, win[c][Wp1]);
-        }
-        const int sk = (k - (z0 - 2)) & (G::NSLOT - 1);
-        const T* pk = ring + sk * G::SLOT;              // plane k: in-plane neighbours
+        for (int c = 0; c < 3; ++c) ldv(pk + c * G::PLANE + own, win[c][W0]);
         T* fb = fbuf + (k & 1) * G::FBUF;
 
         const bool inplane = k < z1;                    // the step past the chunk only needs the z-fluxes
@@ -366,7 +379,6 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
         const Mk hp1z2 = (k + 1 <= N2) ? kAll : kNone, hp1z = (k + 1 <= N2 - 1) ? kAll : kNone;
 
         T fy[3][VEC];       // lower y-fluxes
-        T u0r = T(0);
 
         if (inplane) {
             // y-fluxes: advecting velocity u1 at I and at I - d_i
@@ -379,6 +391,7 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                 ldv(pk + c * G::PLANE + own + G::WX, yp1[c]);
             }
             ld2(pk + G::PLANE + own - 2, u1l);
+            ldv(pkm1 + G::PLANE + own, win[1][Wm1]);
             auto yflux = [&](auto EX_) {
                 constexpr bool EX = decltype(EX_)::value;
                 bool tiny = false;
@@ -421,6 +434,12 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                 T u2l[2], u2d[VEC];                     // u2 at gx-2, gx-1; u2 on row gy-1
                 ld2(pk + 2 * G::PLANE + own - 2, u2l);
                 ldv(pk + 2 * G::PLANE + own - G::WX, u2d);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    ldv(pkm2 + c * G::PLANE + own, win[c][Wm2]);
+                    ldv(pkm1 + c * G::PLANE + own, win[c][Wm1]);
+                    ldv(pkp1 + c * G::PLANE + own, win[c][Wp1]);
+                }
                 auto zflux = [&](auto EX_) {
                     constexpr bool EX = decltype(EX_)::value;
                     bool tiny = false;
@@ -483,7 +502,8 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                 }
                 ldv(pk + own - G::WX, u0d);
                 const T u0ym1_r = pk[own - G::WX + VEC];    // u0 at (gx+VEC, gy-1)
-                u0r = ext[0][VEC + 2];
+                ldv(pkm1 + own, win[0][Wm1]);
+                const T u0r_prev = pkm1[own + VEC];        // u0 at (gx+VEC, gy) on plane k-1
                 __syncwarp();
                 if (lane == 0) mbar_arrive(stepbar);
                 auto xflux = [&](auto EX_) {
@@ -516,9 +536,9 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
             if (lane == 0) mbar_arrive(stepbar);
         }
         if (inplane) {
-            // everybody's y-fluxes of this plane are in fb, and nobody reads slot sk any more
+            // everybody's y-fluxes of this plane are in fb, and nobody reads plane k-2 any more
             mbar_wait(stepbar, (uint32_t)((k - z0) & 1));
-            if (t == 0 && k + 4 <= z1 + 1) issue(k + 4);
+            if (t == 0 && k + 4 <= qlast) issue(k + 4);
             if (full_row) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -529,7 +549,9 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                 }
             }
         }
-        u0r_prev = u0r;
+        s0 = sp1;
+        sp1 = (sp1 + 1 == G::NSLOT) ? 0 : sp1 + 1;
+        if (sp1 == 0) php1 ^= 1u;
     }
 }
 
