@@ -158,6 +158,27 @@ def _algorithmic_bytes_down(n: int, esz: int) -> float:
     return (n + 3 + 1.0 / 2 ** n) * esz
 
 
+# convdiff (NEXT-4), per face flux as the oracle's formula states it: U (2), third-order value (5 incl. the division), limiter
+# bound (3), two medians (8 compare/select), flux (4) = 22 operations; 9 fluxes per 3-D cell (each face flux serves two control
+# volumes) + 2 per flux difference accumulated x 9 = 216 operations per cell (2-D: 4 fluxes, 96).  None can fuse into an FMA
+# (every operation rounds separately, reading 12), so the ALU ceiling is one operation per FP32 lane and clock:
+# SMs x 128 lanes x SM clock (B200_PROFILING.md: 148 SMs; the clock is the one sampled during the run).
+def convdiff_report(cd, n, M, esz, hbm_peak, clocks):
+    if cd is None:
+        return None
+    sec = cd["ms"] * 1e-3
+    nb = 2 * n * esz * M                       # read u, write r: n components each
+    ops = (22 * n * n + 2 * n * n) * M
+    mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965
+    lanes = 128 if esz == 4 else 64            # FP64 units per SM: half the FP32 lanes
+    alu_peak = 148 * lanes * mhz * 1e6 / 1e12
+    return {"kernel": "k_convdiff3d (TMA-staged tiles, every flux once)" if n == 3 else "k_convdiff (one thread per cell)",
+            "ms": cd["ms"], "cells_per_s": M / sec,
+            "roofline": {"bound": "alu", "achieved": ops / sec / 1e12, "peak": alu_peak, "unit": "TFLOP/s", "frac": ops / sec / 1e12 / alu_peak,
+                         "ops_per_cell": ops // M, "peak_source": f"148 SMs x {lanes} lanes x sampled SM clock ({mhz} MHz), one non-fused operation per lane and clock"},
+            "hbm": {"algorithmic_bytes": nb, "achieved_GBps": nb / sec / 1e9, "frac_of_measured": nb / sec / 1e9 / hbm_peak}}
+
+
 def run_reference(args, rank: int):
     """The oracle timed on host cores: each step = one V-cycle (+ mean removal + residual norm) of the same workload."""
     if rank != 0:
@@ -207,6 +228,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-upload-L", action="store_true", help="e2e leg: upload the n·M coefficient array instead of the body records")
     ap.add_argument("--no-pcg", action="store_true", help="skip the conjugate-gradient leg (reported beside the V-cycle solver)")
+    ap.add_argument("--no-convdiff", action="store_true", help="skip the convdiff leg (NEXT-4, timed alone on the same velocity)")
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--graph", type=int, default=1)
     ap.add_argument("--pdl", type=int, default=1, help="WL_OPT_PDL: programmatic dependent launch between the kernels of a cycle")
@@ -345,6 +367,22 @@ def main():
             pcg = {"solver": "wl_solve_pcg (one V-cycle per CG iteration)", "iterations": int(ncp), "converged": bool(rcp == 0),
                    "ms_per_projection": float(np.mean(pms)), "final_rel_residual": float(hp[-1] / hp[0]) if hp[0] > 0 else 0.0}
 
+        # NEXT-4: the other dominant routine of the paper's step (`convdiff!`) on the same velocity field, timed alone
+        cd = None
+        if not args.no_convdiff:
+            rcd = torch.empty_like(u0)
+            for _ in range(3):
+                wl.wl_convdiff(pr.ctx, u0, 1e-3, rcd)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(reps):
+                wl.wl_convdiff(pr.ctx, u0, 1e-3, rcd)
+            e1.record(stream)
+            e1.synchronize()
+            cd = {"ms": e0.elapsed_time(e1) / reps}
+            del rcd
+
         # V-cycles alone: wl_solve with tol = 0 runs exactly `reps` cycles (one graph launch + one 8-byte readback each,
         # mean shift deferred into the next cycle); the dominant kernels alone follow
         if pr.num_levels <= 1:
@@ -404,6 +442,7 @@ def main():
                                 "frac_of_measured": eff / peak, "frac_of_nominal_8TBs": eff / NOMINAL_HBM_GBS})(
             (2 * (n + 3) + 2.0 / 2 ** n) * esz * (2 ** n / (2 ** n - 1.0)) * M / (vcycle_ms * 1e-3) / 1e9),
         "pcg": pcg,
+        "convdiff": convdiff_report(cd, n, M, esz, peak, clocks),
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": roof,

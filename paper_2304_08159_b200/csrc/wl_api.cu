@@ -632,9 +632,12 @@ struct Impl {
     }
 
     // NEXT-4: r = convdiff(u; nu).  Tiled TMA kernel for 3-D grids whose rows are whole 16-byte vectors, else one thread per cell.
+#ifndef WL_CDTY32
+#define WL_CDTY32 11
+#endif
     // rows per tile: fp32 11 + the flux-only row = 12 warps, three per scheduler (measured 512^3: 2.69 ms; 8 rows: 2.96 ms);
     // fp64 8 (256^3: 1.03 ms; 11 rows: 1.19 ms)
-    static constexpr int CDTY = sizeof(T) == 4 ? 11 : 8;
+    static constexpr int CDTY = sizeof(T) == 4 ? WL_CDTY32 : 8;
     static int convdiff(wl_ctx* c, const void* u, double nu, void* r) {
         const Grid& g = c->lev[0].g;
         if constexpr (ND == 3) {
