@@ -319,6 +319,7 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     const Mk wally = (gy == 0 || gy == N1) ? kAll : kNone;
     const Mk hm2y = (gy - 2 >= 0) ? kAll : kNone;
     const Mk hp1y1 = (gy + 1 <= N1) ? kAll : kNone, hp1y = (gy + 1 <= N1 - 1) ? kAll : kNone;
+    const bool y_interior = gy >= 2 && gy + 1 <= N1 - 1;   // warp-uniform: no wall within reach of this row's y-fluxes
     CdConst2 k2;
     if constexpr (VEC == 4) {
         k2.half = f2_pack(0.5f, 0.5f); k2.two = f2_pack(2.0f, 2.0f); k2.five = f2_pack(5.0f, 5.0f); k2.six_neg = f2_pack(-6.0f, -6.0f);
@@ -377,6 +378,7 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
         const Mk wallz = (k == 0 || k == N2) ? kAll : kNone;
         const Mk hm2z = (k - 2 >= 0) ? kAll : kNone;
         const Mk hp1z2 = (k + 1 <= N2) ? kAll : kNone, hp1z = (k + 1 <= N2 - 1) ? kAll : kNone;
+        const bool z_interior = k >= 2 && k + 1 <= N2 - 1;
 
         T fy[3][VEC];       // lower y-fluxes
 
@@ -392,8 +394,10 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
             }
             ld2(pk + G::PLANE + own - 2, u1l);
             ldv(pkm1 + G::PLANE + own, win[1][Wm1]);
-            auto yflux = [&](auto EX_) {
+            auto yflux = [&](auto EX_, auto IN_) {
                 constexpr bool EX = decltype(EX_)::value;
+                constexpr bool IN = decltype(IN_)::value;   // interior row: every flag is a compile-time constant
+                const Mk hm2y_ = IN ? kAll : hm2y, hp1y_ = IN ? kAll : hp1y, hp1y1_ = IN ? kAll : hp1y1, wally_ = IN ? kNone : wally;
                 bool tiny = false;
                 if constexpr (VEC == 4) {
 #pragma unroll
@@ -401,13 +405,13 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                         const u64 a = f2_pack(win[1][W0][e], win[1][W0][e + 1]);
                         const u64 bl = f2_pack((e == 0) ? u1l[1] : win[1][W0][e > 0 ? e - 1 : 0], win[1][W0][e]);
                         cd_flux2<EX>(a, bl, f2_pack(ym2[0][e], ym2[0][e + 1]), f2_pack(ym1[0][e], ym1[0][e + 1]),
-                                     f2_pack(win[0][W0][e], win[0][W0][e + 1]), f2_pack(yp1[0][e], yp1[0][e + 1]), hm2y, hp1y, wally, k2, tiny,
+                                     f2_pack(win[0][W0][e], win[0][W0][e + 1]), f2_pack(yp1[0][e], yp1[0][e + 1]), hm2y_, hp1y_, wally_, k2, tiny,
                                      fy[0][e], fy[0][e + 1]);
                         cd_flux2<EX>(a, f2_pack(ym1[1][e], ym1[1][e + 1]), f2_pack(ym2[1][e], ym2[1][e + 1]), f2_pack(ym1[1][e], ym1[1][e + 1]),
-                                     f2_pack(win[1][W0][e], win[1][W0][e + 1]), f2_pack(yp1[1][e], yp1[1][e + 1]), hm2y, hp1y1, kNone, k2, tiny,
+                                     f2_pack(win[1][W0][e], win[1][W0][e + 1]), f2_pack(yp1[1][e], yp1[1][e + 1]), hm2y_, hp1y1_, kNone, k2, tiny,
                                      fy[1][e], fy[1][e + 1]);
                         cd_flux2<EX>(a, f2_pack(win[1][Wm1][e], win[1][Wm1][e + 1]), f2_pack(ym2[2][e], ym2[2][e + 1]), f2_pack(ym1[2][e], ym1[2][e + 1]),
-                                     f2_pack(win[2][W0][e], win[2][W0][e + 1]), f2_pack(yp1[2][e], yp1[2][e + 1]), hm2y, hp1y, wally, k2, tiny,
+                                     f2_pack(win[2][W0][e], win[2][W0][e + 1]), f2_pack(yp1[2][e], yp1[2][e + 1]), hm2y_, hp1y_, wally_, k2, tiny,
                                      fy[2][e], fy[2][e + 1]);
                     }
                 } else {
@@ -415,14 +419,15 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                     for (int e = 0; e < VEC; ++e) {
                         const T a = win[1][W0][e];
                         const T bl = (e == 0) ? u1l[1] : win[1][W0][e > 0 ? e - 1 : 0];
-                        fy[0][e] = cd_flux<T, EX>(a, bl, ym2[0][e], ym1[0][e], win[0][W0][e], yp1[0][e], hm2y, hp1y, wally, nu, tiny);
-                        fy[1][e] = cd_flux<T, EX>(a, ym1[1][e], ym2[1][e], ym1[1][e], win[1][W0][e], yp1[1][e], hm2y, hp1y1, kNone, nu, tiny);
-                        fy[2][e] = cd_flux<T, EX>(a, win[1][Wm1][e], ym2[2][e], ym1[2][e], win[2][W0][e], yp1[2][e], hm2y, hp1y, wally, nu, tiny);
+                        fy[0][e] = cd_flux<T, EX>(a, bl, ym2[0][e], ym1[0][e], win[0][W0][e], yp1[0][e], hm2y_, hp1y_, wally_, nu, tiny);
+                        fy[1][e] = cd_flux<T, EX>(a, ym1[1][e], ym2[1][e], ym1[1][e], win[1][W0][e], yp1[1][e], hm2y_, hp1y1_, kNone, nu, tiny);
+                        fy[2][e] = cd_flux<T, EX>(a, win[1][Wm1][e], ym2[2][e], ym1[2][e], win[2][W0][e], yp1[2][e], hm2y_, hp1y_, wally_, nu, tiny);
                     }
                 }
                 return tiny;
             };
-            if (yflux(std::false_type{}) && live_y) yflux(std::true_type{});
+            if (y_interior) { if (yflux(std::false_type{}, std::true_type{}) && live_y) yflux(std::true_type{}, std::true_type{}); }
+            else if (yflux(std::false_type{}, std::false_type{}) && live_y) yflux(std::true_type{}, std::false_type{});
             // hand the lower y-fluxes to the row below
 #pragma unroll
             for (int c = 0; c < 3; ++c) stv(fb + (c * G::NW + w) * G::FROW + lane * VEC, fy[c]);
@@ -440,8 +445,10 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                     ldv(pkm1 + c * G::PLANE + own, win[c][Wm1]);
                     ldv(pkp1 + c * G::PLANE + own, win[c][Wp1]);
                 }
-                auto zflux = [&](auto EX_) {
+                auto zflux = [&](auto EX_, auto IN_) {
                     constexpr bool EX = decltype(EX_)::value;
+                    constexpr bool IN = decltype(IN_)::value;   // interior plane
+                    const Mk hm2z_ = IN ? kAll : hm2z, hp1z_ = IN ? kAll : hp1z, hp1z2_ = IN ? kAll : hp1z2, wallz_ = IN ? kNone : wallz;
                     bool tiny = false;
                     if constexpr (VEC == 4) {
 #pragma unroll
@@ -449,13 +456,13 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                             const u64 a = f2_pack(win[2][W0][e], win[2][W0][e + 1]);
                             const u64 bl = f2_pack((e == 0) ? u2l[1] : win[2][W0][e > 0 ? e - 1 : 0], win[2][W0][e]);
                             cd_flux2<EX>(a, bl, f2_pack(win[0][Wm2][e], win[0][Wm2][e + 1]), f2_pack(win[0][Wm1][e], win[0][Wm1][e + 1]),
-                                         f2_pack(win[0][W0][e], win[0][W0][e + 1]), f2_pack(win[0][Wp1][e], win[0][Wp1][e + 1]), hm2z, hp1z, wallz, k2, tiny,
+                                         f2_pack(win[0][W0][e], win[0][W0][e + 1]), f2_pack(win[0][Wp1][e], win[0][Wp1][e + 1]), hm2z_, hp1z_, wallz_, k2, tiny,
                                          fz[0][e], fz[0][e + 1]);
                             cd_flux2<EX>(a, f2_pack(u2d[e], u2d[e + 1]), f2_pack(win[1][Wm2][e], win[1][Wm2][e + 1]), f2_pack(win[1][Wm1][e], win[1][Wm1][e + 1]),
-                                         f2_pack(win[1][W0][e], win[1][W0][e + 1]), f2_pack(win[1][Wp1][e], win[1][Wp1][e + 1]), hm2z, hp1z, wallz, k2, tiny,
+                                         f2_pack(win[1][W0][e], win[1][W0][e + 1]), f2_pack(win[1][Wp1][e], win[1][Wp1][e + 1]), hm2z_, hp1z_, wallz_, k2, tiny,
                                          fz[1][e], fz[1][e + 1]);
                             cd_flux2<EX>(a, f2_pack(win[2][Wm1][e], win[2][Wm1][e + 1]), f2_pack(win[2][Wm2][e], win[2][Wm2][e + 1]), f2_pack(win[2][Wm1][e], win[2][Wm1][e + 1]),
-                                         f2_pack(win[2][W0][e], win[2][W0][e + 1]), f2_pack(win[2][Wp1][e], win[2][Wp1][e + 1]), hm2z, hp1z2, kNone, k2, tiny,
+                                         f2_pack(win[2][W0][e], win[2][W0][e + 1]), f2_pack(win[2][Wp1][e], win[2][Wp1][e + 1]), hm2z_, hp1z2_, kNone, k2, tiny,
                                          fz[2][e], fz[2][e + 1]);
                         }
                     } else {
@@ -463,14 +470,15 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                         for (int e = 0; e < VEC; ++e) {
                             const T a = win[2][W0][e];
                             const T bl = (e == 0) ? u2l[1] : win[2][W0][e > 0 ? e - 1 : 0];
-                            fz[0][e] = cd_flux<T, EX>(a, bl, win[0][Wm2][e], win[0][Wm1][e], win[0][W0][e], win[0][Wp1][e], hm2z, hp1z, wallz, nu, tiny);
-                            fz[1][e] = cd_flux<T, EX>(a, u2d[e], win[1][Wm2][e], win[1][Wm1][e], win[1][W0][e], win[1][Wp1][e], hm2z, hp1z, wallz, nu, tiny);
-                            fz[2][e] = cd_flux<T, EX>(a, win[2][Wm1][e], win[2][Wm2][e], win[2][Wm1][e], win[2][W0][e], win[2][Wp1][e], hm2z, hp1z2, kNone, nu, tiny);
+                            fz[0][e] = cd_flux<T, EX>(a, bl, win[0][Wm2][e], win[0][Wm1][e], win[0][W0][e], win[0][Wp1][e], hm2z_, hp1z_, wallz_, nu, tiny);
+                            fz[1][e] = cd_flux<T, EX>(a, u2d[e], win[1][Wm2][e], win[1][Wm1][e], win[1][W0][e], win[1][Wp1][e], hm2z_, hp1z_, wallz_, nu, tiny);
+                            fz[2][e] = cd_flux<T, EX>(a, win[2][Wm1][e], win[2][Wm2][e], win[2][Wm1][e], win[2][W0][e], win[2][Wp1][e], hm2z_, hp1z2_, kNone, nu, tiny);
                         }
                     }
                     return tiny;
                 };
-                if (zflux(std::false_type{}) && stores) zflux(std::true_type{});
+                if (z_interior) { if (zflux(std::false_type{}, std::true_type{}) && stores) zflux(std::true_type{}, std::true_type{}); }
+                else if (zflux(std::false_type{}, std::false_type{}) && stores) zflux(std::true_type{}, std::false_type{});
                 if (k > z0 && stores) {
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
