@@ -380,10 +380,9 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
         const Mk hp1z2 = (k + 1 <= N2) ? kAll : kNone, hp1z = (k + 1 <= N2 - 1) ? kAll : kNone;
         const bool z_interior = k >= 2 && k + 1 <= N2 - 1;
 
-        T fy[3][VEC];       // lower y-fluxes
-
         if (inplane) {
             // y-fluxes: advecting velocity u1 at I and at I - d_i
+            T fy[3][VEC];       // lower y-fluxes: parked in the exchange buffer, read back when the step's sums are formed
             T ym2[3][VEC], ym1[3][VEC], yp1[3][VEC];    // rows gy-2, gy-1, gy+1
             T u1l[2];                                   // u1 at gx-2, gx-1
 #pragma unroll
@@ -550,10 +549,11 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
             if (full_row) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    T fu[VEC];
+                    T fl[VEC], fu[VEC];
+                    ldv(fb + (c * G::NW + w) * G::FROW + lane * VEC, fl);
                     ldv(fb + (c * G::NW + w + 1) * G::FROW + lane * VEC, fu);
 #pragma unroll
-                    for (int e = 0; e < VEC; ++e) acc[c][e] = acc[c][e] + (fy[c][e] - fu[e]);
+                    for (int e = 0; e < VEC; ++e) acc[c][e] = acc[c][e] + (fl[e] - fu[e]);
                 }
             }
         }
