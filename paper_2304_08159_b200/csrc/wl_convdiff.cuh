@@ -234,7 +234,8 @@ struct CD3 {
     static constexpr int SLOT = 3 * PLANE;
     static constexpr int FROW = TX;              // flux exchange: [2 buffers][3 components][NW rows][TX]
     static constexpr int FBUF = 3 * NW * FROW;
-    static constexpr size_t smem_bytes() { return (size_t)(NSLOT * SLOT + 2 * FBUF) * sizeof(T) + 128 + (NSLOT + 1) * 8; }
+    static constexpr int PARK = 3 * VEC * NT;    // per-thread parking of the carried z-fluxes
+    static constexpr size_t smem_bytes() { return (size_t)(NSLOT * SLOT + 2 * FBUF + PARK) * sizeof(T) + 128 + (NSLOT + 1) * 8; }
 };
 
 template <typename T>
@@ -263,7 +264,9 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     T* ring = reinterpret_cast<T*>(smem_raw);
     T* fbuf = ring + G::NSLOT * G::SLOT;
-    uint64_t* full = reinterpret_cast<uint64_t*>(fbuf + 2 * G::FBUF);
+    const int t_park_off = (int)threadIdx.x * VEC;   // [3][NT][VEC]: conflict-free 16-byte accesses
+    T* park = fbuf + 2 * G::FBUF + t_park_off;
+    uint64_t* full = reinterpret_cast<uint64_t*>(fbuf + 2 * G::FBUF + G::PARK);
     uint64_t* stepbar = full + G::NSLOT;
 
     const int t = threadIdx.x, lane = t & 31, w = t >> 5;
@@ -329,7 +332,6 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
     }
 
     T acc[3][VEC];        // plane k-1: 0 + (x-flux difference) + (y-flux difference), in that order
-    T fzp[3][VEC];        // lower z-flux of plane k-1
     auto ldv = [&](const T* p, T* out) {
         const V v = *reinterpret_cast<const V*>(p);
         if constexpr (VEC == 4) { out[0] = v.x; out[1] = v.y; out[2] = v.z; out[3] = v.w; }
@@ -352,7 +354,7 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int e = 0; e < VEC; ++e) { acc[c][e] = T(0); fzp[c][e] = T(0); }
+        for (int e = 0; e < VEC; ++e) acc[c][e] = T(0);
 
     // One plane step per iteration.  The thread's z-window (its own vector on planes k-2 .. k+1) is read from the ring where it
     // is needed instead of being carried in registers (36 registers and as many moves per step less; carrying it was measured:
@@ -481,10 +483,11 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                 if (k > z0 && stores) {
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
-                        T o[VEC];
+                        T o[VEC], fzp[VEC];               // lower z-flux of plane k-1, parked by the previous step
+                        ldv(park + c * G::NT * VEC, fzp);
 #pragma unroll
                         for (int e = 0; e < VEC; ++e) {
-                            o[e] = acc[c][e] + (fzp[c][e] - fz[c][e]);
+                            o[e] = acc[c][e] + (fzp[e] - fz[c][e]);
                             const bool wallface = (c == 0) ? (gx + e == 0) : (c == 1) ? (gy == 0) : (k - 1 == 0);
                             if (wallface) o[e] = T(0);
                         }
@@ -492,9 +495,7 @@ k_convdiff3d(const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUt
                     }
                 }
 #pragma unroll
-                for (int c = 0; c < 3; ++c)
-#pragma unroll
-                    for (int e = 0; e < VEC; ++e) fzp[c][e] = fz[c][e];
+                for (int c = 0; c < 3; ++c) stv(park + c * G::NT * VEC, fz[c]);
             }
             if (inplane) {
                 // x-fluxes at gx .. gx+VEC: advecting velocity u0 at I and at I - d_i.  These are the last reads of plane k.
