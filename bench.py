@@ -484,6 +484,15 @@ def main():
         tc = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": M * ncyc / tc, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"{ncyc} oracle V-cycle(s) of {cfg['name']} ({tc:.1f} s), host nproc={os.cpu_count()}"}
+        if line.get("convdiff"):
+            # the oracle's convdiff on a bounded sample: the first planes of the same velocity field as a closed box of its own
+            # (same work per cell; about 10 s)
+            us = np.ascontiguousarray(cfg["u"][:, : max(4, min(cfg["u"].shape[1], int(1.6e7 // max(1, M // cfg["u"].shape[1]))))])
+            t0 = time.perf_counter()
+            oracle.convdiff(us, 1e-3)
+            tcd = time.perf_counter() - t0
+            line["convdiff"]["cpu_baseline"] = {"value": us[0].size / tcd, "unit": "cells/s", "cores": 1, "kind": "oracle",
+                                                "sample": f"oracle convdiff on the first {us.shape[1]} planes of {cfg['name']} ({tcd:.1f} s)"}
     if rank == 0:
         print(json.dumps(line), flush=True)
     pr.close()
