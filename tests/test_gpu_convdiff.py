@@ -141,6 +141,28 @@ def test_convdiff_is_reproducible_run_to_run(env):
         pr.close()
 
 
+def test_convdiff_misaligned_arrays_take_the_any_shape_kernel(env):
+    """Caller arrays that do not start on a 16-byte boundary (a slice of a larger tensor) cannot be TMA sources: the call must
+    fall back to the one-thread-per-cell kernel, not fail, and give the same field."""
+    torch, wl = env["torch"], env["wl"]
+    dims = (136, 24, 20)
+    u = _field(dims, np.float32, 3, "smooth")
+    ref = env["oracle"].convdiff(u, 0.02)
+    pr = wl.Projector(dims, np.float32)
+    n = u.size
+    ubuf = torch.zeros(n + 4, dtype=torch.float32, device="cuda")
+    rbuf = torch.full((n + 4,), float("nan"), dtype=torch.float32, device="cuda")
+    ud = ubuf[1:1 + n].view(u.shape)
+    rd = rbuf[3:3 + n].view(u.shape)
+    assert ud.data_ptr() % 16 != 0 and rd.data_ptr() % 16 != 0
+    ud.copy_(torch.from_numpy(u))
+    wl.wl_convdiff(pr.ctx, ud, 0.02, rd)
+    torch.cuda.synchronize()
+    assert np.array_equal(rd.cpu().numpy(), ref)
+    assert torch.isnan(rbuf[:3]).all() and torch.isnan(rbuf[3 + n:]).all()      # nothing written outside the field
+    pr.close()
+
+
 def test_convdiff_argument_errors(env):
     torch, wl = env["torch"], env["wl"]
     pr = wl.Projector((16, 8, 8), np.float32)
