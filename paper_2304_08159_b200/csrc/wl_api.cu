@@ -569,6 +569,13 @@ struct Impl {
     // ---- V-cycle-preconditioned conjugate gradients (wl_pcg.cuh) ------------------------------------
     static int pcg_residual(wl_ctx* c, const void* x, const void* b) {
         Level& f = c->lev[0];
+        if (rows_ok(f.g, f.L, x, b)) {
+            const int gr = rows_grid(c, (long long)f.g.N1 * f.g.N2);
+            k_pcg_Ap_rows<T, ND, true><<<gr, dim3(kRowsX, kRowsY), 0, c->stream>>>(f.g, P(f.L), P(x), P(c->cg_v[0]), c->d_scal, c->d_partials, P(b),
+                                                                                  c->d_hist, c->h_scal, c->h_hist);
+            KCHECK(c, "k_pcg_Ap_rows");
+            return WL_OK;
+        }
         k_pcg_residual<T, ND><<<nparts_for(c, f.g.M), kBlock, 0, c->stream>>>(f.g, P(f.L), P(x), P(b), P(c->cg_v[0]), c->d_scal, c->d_hist,
                                                                            c->h_scal, c->h_hist);
         KCHECK(c, "k_pcg_residual");
@@ -584,11 +591,24 @@ struct Impl {
         const int np = nparts_for(c, M) < kMaxPartials / 2 ? nparts_for(c, M) : kMaxPartials / 2;
         k_pcg_dot_rz<T><<<np, kBlock, 0, c->stream>>>(M, r, z, c->d_scal, c->d_partials);
         KCHECK(c, "k_pcg_dot_rz");
-        k_pcg_update_p<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, z, p, c->d_scal);
-        KCHECK(c, "k_pcg_update_p");
-        k_pcg_Ap<T, ND><<<np, kBlock, 0, c->stream>>>(f.g, P(f.L), p, q, c->d_scal, c->d_partials);
-        KCHECK(c, "k_pcg_Ap");
-        k_pcg_update_xr<T><<<np, kBlock, 0, c->stream>>>(M, P(x), r, p, q, c->d_scal, c->d_hist, c->h_scal, c->h_hist);
+        const bool vec = rows_ok(f.g, x, nullptr, nullptr);   // the work vectors are the context's own (aligned); x is the caller's
+        if (vec) {
+            k_pcg_update_p_vec<T><<<grid_for(c, M / (16 / (long long)sizeof(T))), kBlock, 0, c->stream>>>(M, z, p, c->d_scal);
+            KCHECK(c, "k_pcg_update_p_vec");
+        } else {
+            k_pcg_update_p<T><<<grid_for(c, M), kBlock, 0, c->stream>>>(M, z, p, c->d_scal);
+            KCHECK(c, "k_pcg_update_p");
+        }
+        if (rows_ok(f.g, f.L, p, q)) {
+            const int gr = rows_grid(c, (long long)f.g.N1 * f.g.N2);
+            k_pcg_Ap_rows<T, ND, false><<<gr < kMaxPartials ? gr : kMaxPartials, dim3(kRowsX, kRowsY), 0, c->stream>>>(f.g, P(f.L), p, q, c->d_scal, c->d_partials, nullptr, nullptr, nullptr, nullptr);
+            KCHECK(c, "k_pcg_Ap_rows");
+        } else {
+            k_pcg_Ap<T, ND><<<np, kBlock, 0, c->stream>>>(f.g, P(f.L), p, q, c->d_scal, c->d_partials);
+            KCHECK(c, "k_pcg_Ap");
+        }
+        if (vec) k_pcg_update_xr<T, true><<<np, kBlock, 0, c->stream>>>(M, P(x), r, p, q, c->d_scal, c->d_hist, c->h_scal, c->h_hist);
+        else k_pcg_update_xr<T, false><<<np, kBlock, 0, c->stream>>>(M, P(x), r, p, q, c->d_scal, c->d_hist, c->h_scal, c->h_hist);
         KCHECK(c, "k_pcg_update_xr");
         return WL_OK;
     }
@@ -632,12 +652,9 @@ struct Impl {
     }
 
     // NEXT-4: r = convdiff(u; nu).  Tiled TMA kernel for 3-D grids whose rows are whole 16-byte vectors, else one thread per cell.
-#ifndef WL_CDTY32
-#define WL_CDTY32 11
-#endif
     // rows per tile: fp32 11 + the flux-only row = 12 warps, three per scheduler (measured 512^3: 2.69 ms; 8 rows: 2.96 ms);
     // fp64 8 (256^3: 1.03 ms; 11 rows: 1.19 ms)
-    static constexpr int CDTY = sizeof(T) == 4 ? WL_CDTY32 : 8;
+    static constexpr int CDTY = sizeof(T) == 4 ? 11 : 8;
     static int convdiff(wl_ctx* c, const void* u, double nu, void* r) {
         const Grid& g = c->lev[0].g;
         if constexpr (ND == 3) {

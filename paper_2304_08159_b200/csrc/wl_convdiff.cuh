@@ -13,9 +13,10 @@
 //
 // Two kernels: k_convdiff (any shape, 2-D / 3-D, one thread per cell, every flux evaluated by both cells it separates) and
 // k_convdiff3d (3-D, rows of whole 16-byte vectors): a CTA owns a 32·VEC x TY tile and marches along z; planes arrive by TMA
-// (zero fill beyond the box = the unstored upper wall values), a thread owns one 16-byte vector of one row and keeps its four-
-// plane z-window in registers, every flux is evaluated ONCE (x: 4+1 per thread, y: handed to the row below through shared
-// memory, z: carried to the next plane in registers).
+// into a six-slot ring (zero fill beyond the box = the unstored upper wall values; planes k-2 .. k+1 are read from the ring, two
+// more are in flight); a warp is one row, a thread owns one 16-byte vector of it; every flux is evaluated ONCE (x: 4+1 per
+// thread; y: handed to the row below through shared memory, one more warp evaluates the row above the tile; z: the lower-face
+// flux of plane k completes plane k-1 and is parked in shared memory for the next step).  DESIGN.md §6.6 has the measurements.
 #pragma once
 #include <cuda.h>
 

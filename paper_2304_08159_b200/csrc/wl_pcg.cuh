@@ -12,6 +12,7 @@
 #pragma once
 #include "wl_common.cuh"
 #include "wl_generic.cuh"
+#include "wl_rows.cuh"
 
 namespace wl {
 
@@ -128,6 +129,27 @@ __global__ void k_pcg_update_p(long long M, const T* __restrict__ z, T* __restri
     }
 }
 
+// the same with 16-byte accesses (M a multiple of the vector width, aligned arrays)
+template <typename T>
+__global__ void k_pcg_update_p_vec(long long M, const T* __restrict__ z, T* __restrict__ p, const Scalars* __restrict__ scal) {
+    if (scal->done || scal->breakdown) return;
+    constexpr int VEC = 16 / (int)sizeof(T);
+    const T mz = (T)scal->mean_p, beta = (T)scal->beta;
+    const long long nv = M / VEC;
+    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < nv; v += (long long)gridDim.x * blockDim.x) {
+        T zv[VEC], pv[VEC];
+        ld_vec<T, VEC>(z + v * VEC, zv);
+        ld_vec<T, VEC>(p + v * VEC, pv);
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) {
+            const T zs = zv[k] - mz;
+            const T bp = beta * pv[k];
+            pv[k] = zs + bp;
+        }
+        st_vec<T, VEC>(p + v * VEC, pv);
+    }
+}
+
 // q = A p, sigma = sum p q; alpha = rho / sigma
 template <typename T, int ND>
 __global__ void k_pcg_Ap(Grid g, const T* __restrict__ L, const T* __restrict__ p, T* __restrict__ q, Scalars* scal,
@@ -154,9 +176,111 @@ __global__ void k_pcg_Ap(Grid g, const T* __restrict__ L, const T* __restrict__ 
     }
 }
 
+// The same as a row kernel (16-byte loads along the unit-stride axis, two integer divisions per row instead of per cell; rows
+// of whole vectors, aligned arrays).  Per cell the terms and their order are stencil_cell's: upper face, lower face; axis 0, 1, 2.
+// RESID: q = b - A p and ||q||inf -> hist[0] with the first stop decision (k_pcg_residual) instead of q = A p, sigma, alpha.
+template <typename T, int ND, bool RESID>
+__global__ void __launch_bounds__(kRowsX* kRowsY) k_pcg_Ap_rows(Grid g, const T* __restrict__ L, const T* __restrict__ p,
+                                                               T* __restrict__ q, Scalars* scal, double* __restrict__ partials,
+                                                               const T* __restrict__ b, double* hist, Scalars* host_mirror,
+                                                               double* host_hist) {
+    if (!RESID && (scal->done || scal->breakdown)) return;
+    constexpr int VEC = 16 / (int)sizeof(T);
+    __shared__ double red[32];
+    const int nvx = g.N0 / VEC;
+    const long long nrows = (long long)g.N1 * g.N2;
+    const long long sy = g.N0, sz = (long long)g.N0 * g.N1;
+    const T* L0 = L;
+    const T* L1 = L + g.M;
+    const T* L2 = L + 2 * g.M;
+    double s = 0.0;
+    for (long long r = (long long)blockIdx.x * kRowsY + threadIdx.y; r < nrows; r += (long long)gridDim.x * kRowsY) {
+        const int z = (int)(r / g.N1), y = (int)(r - (long long)z * g.N1);
+        const bool up1 = y + 1 < g.N1, lo1 = y > 0, up2 = (ND == 3) && (z + 1 < g.N2), lo2 = (ND == 3) && (z > 0);
+        for (int vx = threadIdx.x; vx < nvx; vx += kRowsX) {
+            const int x = vx * VEC;
+            const long long e0 = r * g.N0 + x;
+            T pc[VEC], l0[VEC], l1[VEC], l1u[VEC], py_u[VEC], py_l[VEC], out[VEC];
+            ld_vec<T, VEC>(p + e0, pc);
+            ld_vec<T, VEC>(L0 + e0, l0);
+            ld_vec<T, VEC>(L1 + e0, l1);
+            T bv[VEC];
+            if (RESID) ld_vec<T, VEC>(b + e0, bv);
+            const bool upx = x + VEC < g.N0;
+            const T pxn = upx ? p[e0 + VEC] : (T)0, l0n = upx ? L0[e0 + VEC] : (T)0;
+            const T pxm = (x > 0) ? p[e0 - 1] : (T)0;
+            if (up1) { ld_vec<T, VEC>(p + e0 + sy, py_u); ld_vec<T, VEC>(L1 + e0 + sy, l1u); }
+            if (lo1) ld_vec<T, VEC>(p + e0 - sy, py_l);
+            T l2[VEC], l2u[VEC], pz_u[VEC], pz_l[VEC];
+            if (ND == 3) {
+                ld_vec<T, VEC>(L2 + e0, l2);
+                if (up2) { ld_vec<T, VEC>(p + e0 + sz, pz_u); ld_vec<T, VEC>(L2 + e0 + sz, l2u); }
+                if (lo2) ld_vec<T, VEC>(p + e0 - sz, pz_l);
+            }
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) {
+                const T xc = pc[k];
+                T a = 0;
+                if (k + 1 < VEC) a += l0[(k + 1) % VEC] * (pc[(k + 1) % VEC] - xc);
+                else if (upx) a += l0n * (pxn - xc);
+                if (k > 0) a += l0[k] * (pc[(k + VEC - 1) % VEC] - xc);
+                else if (x > 0) a += l0[k] * (pxm - xc);
+                if (up1) a += l1u[k] * (py_u[k] - xc);
+                if (lo1) a += l1[k] * (py_l[k] - xc);
+                if (ND == 3) {
+                    if (up2) a += l2u[k] * (pz_u[k] - xc);
+                    if (lo2) a += l2[k] * (pz_l[k] - xc);
+                }
+                if (RESID) {
+                    out[k] = bv[k] - a;
+                    s = nanmax(s, fabs((double)out[k]));
+                } else {
+                    out[k] = a;
+                    s += (double)xc * (double)a;
+                }
+            }
+            st_vec<T, VEC>(q + e0, out);
+        }
+    }
+    {   // CTA sum (thread index is two-dimensional here), partial, ordered second stage by the last CTA
+        const int tid = threadIdx.y * kRowsX + threadIdx.x;
+        s = RESID ? warp_max(s) : warp_sum(s);
+        if ((tid & 31) == 0) red[tid >> 5] = s;
+        __syncthreads();
+        if (tid < 32) {
+            s = (tid < (kRowsX * kRowsY) / 32) ? red[tid] : 0.0;
+            s = RESID ? warp_max(s) : warp_sum(s);
+            if (tid == 0) {
+                if (RESID) atomic_max_nonneg(&scal->absmax_bits[1], s);
+                else partials[blockIdx.x] = s;
+            }
+        }
+    }
+    __shared__ int s_last;
+    __syncthreads();
+    const int tid = threadIdx.y * kRowsX + threadIdx.x;
+    if (tid == 0) {
+        __threadfence();
+        const unsigned int ticket = atomicAdd(&scal->ticket, 1u);
+        s_last = (ticket == gridDim.x - 1) ? 1 : 0;
+        if (s_last) scal->ticket = 0u;
+    }
+    __syncthreads();
+    if (RESID) {
+        if (s_last && tid == 0) { __threadfence(); pcg_record(scal, hist, host_mirror, host_hist); }
+    } else if (s_last && tid < 32) {
+        __threadfence();
+        const double sigma = ordered_sum(partials, (int)gridDim.x, 1);
+        if (tid == 0) {
+            if (sigma == 0.0) scal->breakdown = 1;
+            else scal->alpha = scal->rho / sigma;
+        }
+    }
+}
+
 // x += alpha p, r -= alpha q, ||r||inf -> hist[k+1], stop decision.  A breakdown (rho' = 0 or sigma = 0: nothing left to
 // correct) ends the solve as converged without touching x.
-template <typename T>
+template <typename T, bool VECTOR>
 __global__ void k_pcg_update_xr(long long M, T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
                                 const T* __restrict__ q, Scalars* scal, double* hist, Scalars* host_mirror, double* host_hist) {
     if (scal->done) return;
@@ -165,6 +289,27 @@ __global__ void k_pcg_update_xr(long long M, T* __restrict__ x, T* __restrict__ 
     double m = 0.0;
     if (!brk) {
         const T alpha = (T)scal->alpha;
+        if (VECTOR) {   // 16-byte accesses (M a multiple of the vector width, aligned arrays)
+            constexpr int VEC = 16 / (int)sizeof(T);
+            const long long nv = M / VEC;
+            for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < nv; v += (long long)gridDim.x * blockDim.x) {
+                T xv[VEC], rv[VEC], pv[VEC], qv[VEC];
+                ld_vec<T, VEC>(x + v * VEC, xv);
+                ld_vec<T, VEC>(p + v * VEC, pv);
+                ld_vec<T, VEC>(r + v * VEC, rv);
+                ld_vec<T, VEC>(q + v * VEC, qv);
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    const T ap = alpha * pv[k];
+                    xv[k] = xv[k] + ap;
+                    const T aq = alpha * qv[k];
+                    rv[k] = rv[k] - aq;
+                    m = nanmax(m, fabs((double)rv[k]));
+                }
+                st_vec<T, VEC>(x + v * VEC, xv);
+                st_vec<T, VEC>(r + v * VEC, rv);
+            }
+        } else
         for (long long I = (long long)blockIdx.x * blockDim.x + threadIdx.x; I < M; I += (long long)gridDim.x * blockDim.x) {
             const T ap = alpha * p[I];
             x[I] = x[I] + ap;
