@@ -90,6 +90,7 @@ struct wl_ctx {
     bool unaligned = false;      // a caller array of the running call is not 16-byte aligned: no TMA on its level
     int unaligned_level = 0;
     int tail_first = kMaxLevels; // first level of the single-CTA coarse tail (>= nlev: none fits shared memory)
+    int pcg_up = 0;              // set while enqueuing z = V(r) of a CG iteration whose level-0 UP kernel also forms r·z and beta
     int check_done = 0;          // set while enqueuing a solve cycle: kernels that can, return at once when scal->done
     int fused_grid = 0;          // CTAs of the last fused launch (= number of sum partials it wrote)
     int64_t launches = 0;
@@ -396,6 +397,7 @@ struct Impl {
             prm.cells = f.g.M;
             prm.negzero2 = 0x8000000080000000ULL;
             prm.check_done = c->check_done;
+            prm.pcg = (NORMS && c->pcg_up) ? 1 : 0;
             auto kern = k_fused3d<T, FTX, FTY, FPF<PROLONG>, PROLONG, ZERO_IN, SHIFT, STAGE3, RESTRICT, NORMS, RIN, USEC, TICKET>;
             constexpr size_t smem = fused3d_smem_bytes<T, FTX, FTY, FPF<PROLONG>, PROLONG, USEC>();
             const int g = f.plan_grid;
@@ -420,7 +422,7 @@ struct Impl {
     // UP half of level l: x_out = J(J(x_in + P xc)).
     static int up(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out) {
         if (!fused_ok(c, l)) return up_generic(c, l, x_in, xc, b, x_out);
-        if (c->opt_solve_kernels && l == 0 && c->d_hist)
+        if ((c->opt_solve_kernels || c->pcg_up) && l == 0 && c->d_hist)
             return launch_fused<true, false, false, false, false, true, false, true>(c, l, x_in, xc, b, x_out, nullptr);
         return launch_fused<true, false, false, false, false, false>(c, l, x_in, xc, b, x_out, nullptr);
     }
@@ -587,10 +589,17 @@ struct Impl {
         const long long M = f.g.M;
         T* r = P(c->cg_v[0]); T* z = P(c->cg_v[1]); T* p = P(c->cg_v[2]); T* q = P(c->cg_v[3]);
         int rc;
-        if ((rc = vcycle(c, 0, nullptr, r, f.x[1], z))) return rc;
+        // with a fused 3-D level 0 the last kernel of the V-cycle (level-0 UP) also forms sum z, sum r z and beta
+        const bool dot_in_up = ND == 3 && c->nlev > 1 && c->tail_first > 0 && fused_ok(c, 0) && c->d_hist;
+        c->pcg_up = dot_in_up ? 1 : 0;
+        rc = vcycle(c, 0, nullptr, r, f.x[1], z);
+        c->pcg_up = 0;
+        if (rc) return rc;
         const int np = nparts_for(c, M) < kMaxPartials / 2 ? nparts_for(c, M) : kMaxPartials / 2;
-        k_pcg_dot_rz<T><<<np, kBlock, 0, c->stream>>>(M, r, z, c->d_scal, c->d_partials);
-        KCHECK(c, "k_pcg_dot_rz");
+        if (!dot_in_up) {
+            k_pcg_dot_rz<T><<<np, kBlock, 0, c->stream>>>(M, r, z, c->d_scal, c->d_partials);
+            KCHECK(c, "k_pcg_dot_rz");
+        }
         const bool vec = rows_ok(f.g, x, nullptr, nullptr);   // the work vectors are the context's own (aligned); x is the caller's
         if (vec) {
             k_pcg_update_p_vec<T><<<grid_for(c, M / (16 / (long long)sizeof(T))), kBlock, 0, c->stream>>>(M, z, p, c->d_scal);

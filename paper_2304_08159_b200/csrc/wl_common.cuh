@@ -124,4 +124,27 @@ __device__ __forceinline__ void solve_finish_mean_lagged(Scalars* scal, const do
     }
 }
 
+// ordered sum of nparts partials with stride `stride` doubles, by one warp (lane l adds l, l+32, ...; shuffle tree)
+__device__ __forceinline__ double ordered_sum(const double* partials, int nparts, int stride) {
+    const int lane = threadIdx.x & 31;
+    double s = 0.0;
+    for (int i = lane; i < nparts; i += 32) s += ((const volatile double*)partials)[(size_t)i * stride];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    return __shfl_sync(0xffffffffu, s, 0);
+}
+
+// Conjugate-gradient bookkeeping after z = V(r) (wl_pcg.cuh): partials hold per-CTA (sum z, sum r z) pairs; mean of z, beta =
+// rho'/rho (0 on the first iteration), rho <- rho'; rho' = 0 ends the solve.  One warp (all 32 lanes must call).
+__device__ __forceinline__ void pcg_finish_dot(Scalars* scal, const double* partials, int nparts, long long M) {
+    const double tz = ordered_sum(partials, nparts, 2);
+    const double trz = ordered_sum(partials + 1, nparts, 2);
+    if ((threadIdx.x & 31) == 0) {
+        scal->mean_p = tz / (double)M;                       // mz
+        scal->beta = (scal->cycle == 0 || scal->rho == 0.0) ? 0.0 : trz / scal->rho;
+        scal->rho = trz;
+        if (trz == 0.0) scal->breakdown = 1;
+    }
+}
+
 }  // namespace wl

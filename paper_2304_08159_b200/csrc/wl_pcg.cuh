@@ -16,16 +16,6 @@
 
 namespace wl {
 
-// ordered sum of nparts partials with stride `stride` doubles, by one warp (lane l adds l, l+32, ...; shuffle tree)
-__device__ __forceinline__ double ordered_sum(const double* partials, int nparts, int stride) {
-    const int lane = threadIdx.x & 31;
-    double s = 0.0;
-    for (int i = lane; i < nparts; i += 32) s += ((const volatile double*)partials)[(size_t)i * stride];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
-    return __shfl_sync(0xffffffffu, s, 0);
-}
-
 // true in every thread of the last CTA of the launch to get here (after publishing its partials), false elsewhere
 __device__ __forceinline__ bool last_cta(Scalars* scal) {
     __shared__ int s_last;
@@ -105,16 +95,7 @@ __global__ void k_pcg_dot_rz(long long M, const T* __restrict__ r, const T* __re
     sz = block_sum(sz, red);
     srz = block_sum(srz, red);
     if (threadIdx.x == 0) { partials[2 * blockIdx.x] = sz; partials[2 * blockIdx.x + 1] = srz; }
-    if (last_cta(scal) && threadIdx.x < 32) {
-        const double tz = ordered_sum(partials, (int)gridDim.x, 2);
-        const double trz = ordered_sum(partials + 1, (int)gridDim.x, 2);
-        if (threadIdx.x == 0) {
-            scal->mean_p = tz / (double)M;                       // mz
-            scal->beta = (scal->cycle == 0 || scal->rho == 0.0) ? 0.0 : trz / scal->rho;
-            scal->rho = trz;
-            if (trz == 0.0) scal->breakdown = 1;
-        }
-    }
+    if (last_cta(scal) && threadIdx.x < 32) pcg_finish_dot(scal, partials, (int)gridDim.x, M);
 }
 
 // p = (z - mz) + beta p
