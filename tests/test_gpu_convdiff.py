@@ -13,7 +13,7 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 
-SHAPES = [(8, 8, 8), (12, 10, 6), (128, 8, 8), (136, 24, 20), (256, 40, 12), (64, 64, 64), (132, 17, 9), (16, 4, 4),
+SHAPES = [(8, 8, 8), (12, 10, 6), (128, 8, 8), (136, 24, 20), (256, 40, 12), (64, 64, 64), (132, 17, 9), (16, 4, 4), (128, 64, 64),
           (13, 9, 7), (6, 5, 4), (64, 64), (33, 17), (256, 24)]
 DTYPES = [np.float32, np.float64]
 
