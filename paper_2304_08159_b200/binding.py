@@ -45,6 +45,8 @@ SIGNATURES = {
     "wl_up": (_i32, [_vp, _i32, _vp, _vp, _vp, _vp]),
     "wl_vcycle_level": (_i32, [_vp, _i32, _vp, _vp]),
     "wl_residual_norm": (_i32, [_vp, _vp, _vp, _f64p, _f64p]),
+    "wl_residual_norm_static": (_i32, [_i32, _i64p, _i32, _vp, _vp, _vp, _vp, _vp]),
+    "wl_static_last_error": (ctypes.c_char_p, []),
     "wl_num_levels": (_i32, [_vp]),
     "wl_level_dims": (_i32, [_vp, _i32, _i64p]),
     "wl_get_coeff": (_i32, [_vp, _i32, _vp]),
@@ -240,6 +242,36 @@ def wl_residual_norm(ctx, p, b):
     r, m = ctypes.c_double(0.0), ctypes.c_double(0.0)
     _check(ctx, load().wl_residual_norm(ctx, _dptr(p), _dptr(b), ctypes.byref(r), ctypes.byref(m)), "wl_residual_norm")
     return r.value, m.value
+
+
+WL_STATIC_MAX_CELLS = 1 << 27
+
+
+def wl_residual_norm_static(dims, L, p, b, out, stream=None):
+    """Context-free residual check that allocates nothing on the device (include/wl.h): for a caller who has no device
+    memory left to request, or no allocator of its own, in the middle of a run.  dims = (N_0,…,N_{n-1}) as in wl_create;
+    L, p, b: CUDA tensors of one dtype; out: CUDA float64 tensor of >= 2 elements, receives (||b - A p||inf, mean(p)) when
+    the stream has drained.  Enqueued on `stream` (default: torch's current stream).  Grids above WL_STATIC_MAX_CELLS are
+    refused.  Calls on one GPU share a fixed scratch array: keep them in stream order."""
+    import torch
+    if out.dtype != torch.float64 or out.numel() < 2:
+        raise ValueError("out must be a float64 CUDA tensor of at least 2 elements")
+    if not (L.dtype == p.dtype == b.dtype):
+        raise ValueError("L, p, b must share one dtype")
+    n = len(dims)
+    arr = (ctypes.c_int64 * max(n, 1))(*[int(d) for d in dims])
+    s = torch.cuda.current_stream(p.device) if stream is None else stream
+    lib = load()
+    with torch.cuda.device(p.device):                      # the scratch address is looked up for the CURRENT device
+        rc = lib.wl_residual_norm_static(n, arr, _dtype_code(p.dtype), _dptr(L), _dptr(p), _dptr(b), _dptr(out),
+                                         ctypes.c_void_p(s.cuda_stream))
+    if rc < 0:
+        raise WlError(rc, "wl_residual_norm_static", (lib.wl_static_last_error() or b"").decode())
+    return rc
+
+
+def wl_static_last_error() -> str:
+    return (load().wl_static_last_error() or b"").decode()
 
 
 def wl_num_levels(ctx) -> int:
