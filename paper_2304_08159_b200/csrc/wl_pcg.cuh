@@ -57,6 +57,7 @@ __global__ void k_pcg_begin(Scalars* scal, double tol, int maxit) {
         scal->shift = 0.0;
         scal->done = 0;
         scal->rho = 0.0;
+        scal->breakdown = 0;   // a breakdown of an earlier solve (e.g. an all-solid field, z = 0) must not end this one
     }
 }
 
