@@ -36,10 +36,14 @@
 //                  value of the paper.
 //
 //   body_coeff     (the BDIM! row of Table 2)
-//                  pinned: mu0(-1) = 0, mu0(0) = 1/2, mu0(1) = 1, mu0(d) + mu0(-d) = 1, monotone, C^1 at
-//                  +-1 (derivative 0); exact 0 / 1 at faces farther than one cell inside / outside a body;
-//                  the cell-integral of 1 - L over a sphere reproduces its volume; face-centre
-//                  convention checked on a half-space-like huge sphere (tests/test_oracle_body.py).
+//                  pinned (tests/test_oracle_body.py): mu0(-1) = 0, mu0(0) = 1/2, mu0(1) = 1, the closed forms
+//                  mu0(+-1/2) = 1/2 +- (1/4 + 1/(2 pi)), mu0(d) + mu0(-d) = 1, monotone, contact with 0 and 1
+//                  at +-1 (1e-11 at 1e-4 inside), never negative just inside d = -1; exact 0 / 1 at faces
+//                  farther than one cell inside / outside a body and 0 on the stored wall planes; the
+//                  face-centre convention on a radius-1/2 sphere centred ON a face centre (closed-form
+//                  distances of the neighbouring face centres); the lattice sum of 1 - L over each face
+//                  family against 4/3 pi R^3 + 4 pi R (1/3 - 2/pi^2); several bodies = the minimum distance;
+//                  a torus with faces exactly on its surface, centre line and one cell outside.
 //
 //   convdiff       (`convdiff!`; "third-order finite volume")
 //                  pinned: the face value against Leonard's normalised-variable diagram written independently, exact
