@@ -47,6 +47,7 @@ SIGNATURES = {
     "wl_residual_norm": (_i32, [_vp, _vp, _vp, _f64p, _f64p]),
     "wl_residual_norm_static": (_i32, [_i32, _i64p, _i32, _vp, _vp, _vp, _vp, _vp]),
     "wl_static_last_error": (ctypes.c_char_p, []),
+    "wl_selftest_recip": (_i32, [_vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint32)]),
     "wl_num_levels": (_i32, [_vp]),
     "wl_level_dims": (_i32, [_vp, _i32, _i64p]),
     "wl_get_coeff": (_i32, [_vp, _i32, _vp]),
@@ -242,6 +243,13 @@ def wl_residual_norm(ctx, p, b):
     r, m = ctypes.c_double(0.0), ctypes.c_double(0.0)
     _check(ctx, load().wl_residual_norm(ctx, _dptr(p), _dptr(b), ctypes.byref(r), ctypes.byref(m)), "wl_residual_norm")
     return r.value, m.value
+
+
+def wl_selftest_recip(ctx):
+    """Exhaustive device check of the fused kernels' fp32 reciprocal against IEEE 1/d.  Returns (mismatches, first bad bits)."""
+    n, first = ctypes.c_uint64(0), ctypes.c_uint32(0)
+    _check(ctx, load().wl_selftest_recip(ctx, ctypes.byref(n), ctypes.byref(first)), "wl_selftest_recip")
+    return int(n.value), int(first.value)
 
 
 WL_STATIC_MAX_CELLS = 1 << 27

@@ -62,6 +62,8 @@ struct wl_ctx {
     int hist_cap = 0;
     void* b0 = nullptr;          // ctx-owned right-hand side for wl_project
     double* d_bodies = nullptr;  // device copy of the body records of wl_set_bodies
+    double* h_bodies = nullptr;  // pinned staging copy of the caller's records: the caller may rewrite its array as soon as the call returns
+    cudaEvent_t ev_bodies = nullptr;   // the upload out of h_bodies has completed
     void* cg_v[4] = {nullptr, nullptr, nullptr, nullptr};   // r, z, p, q of the conjugate-gradient solve (allocated on first use)
     int opt_solver = 0;          // WL_OPT_SOLVER: 0 = V-cycles (BJ), 1 = V-cycle-preconditioned CG (NEXT-1)
     void* stage_u = nullptr;     // device staging for wl_project_host
@@ -72,6 +74,8 @@ struct wl_ctx {
     int opt_host_p_zero = 0;     // WL_OPT_HOST_P_ZERO: wl_project_host starts from p = 0 without uploading p_host
     bool have_coeff = false;
     int opt_fused = 1, opt_graph = 1, opt_coarse_cta = 1, opt_solve_kernels = 0;
+    int solve_kernels_now = 0;   // WL_OPT_SOLVE_KERNELS applies to the wl_down / wl_up ENTRY POINTS only: set for the length of such a
+                                 // call, so that the V-cycles of wl_vcycle / wl_solve / wl_solve_pcg never pick those instances up
     int opt_pdl = 1;             // WL_OPT_PDL: chain the cycle's kernels by programmatic dependent launch
     bool pdl_armed = false;      // the last launch enqueued by the running call was a kernel that waits before touching data
     int num_sms = 148;
@@ -413,7 +417,7 @@ struct Impl {
     // DOWN half of level l: x_out = J(J(x_in)) (x_in == nullptr: from zero), bc = R(b - A x_out).
     static int down(wl_ctx* c, int l, const void* x_in, const void* b, void* x_out, void* bc) {
         if (!fused_ok(c, l)) return down_generic(c, l, x_in, b, x_out, bc);
-        if (c->opt_solve_kernels && l == 0 && x_in && c->d_hist)   // the instance wl_solve's graph launches (profiling / bench)
+        if (c->solve_kernels_now && l == 0 && x_in && c->d_hist)   // the instance wl_solve's graph launches (profiling / bench)
             return launch_fused<false, false, true, true, true, false, true, true>(c, l, x_in, nullptr, b, x_out, bc);
         if (x_in) return launch_fused<false, false, false, true, true, false>(c, l, x_in, nullptr, b, x_out, bc);
         return launch_fused<false, true, false, true, true, false>(c, l, nullptr, nullptr, b, x_out, bc);
@@ -422,7 +426,7 @@ struct Impl {
     // UP half of level l: x_out = J(J(x_in + P xc)).
     static int up(wl_ctx* c, int l, const void* x_in, const void* xc, const void* b, void* x_out) {
         if (!fused_ok(c, l)) return up_generic(c, l, x_in, xc, b, x_out);
-        if ((c->opt_solve_kernels || c->pcg_up) && l == 0 && c->d_hist)
+        if ((c->solve_kernels_now || c->pcg_up) && l == 0 && c->d_hist)
             return launch_fused<true, false, false, false, false, true, false, true>(c, l, x_in, xc, b, x_out, nullptr);
         return launch_fused<true, false, false, false, false, false>(c, l, x_in, xc, b, x_out, nullptr);
     }
@@ -1116,6 +1120,8 @@ void wl_destroy(wl_ctx* c) {
     if (c->h_scal) cudaFreeHost(c->h_scal);
     if (c->b0) cudaFree(c->b0);
     if (c->d_bodies) cudaFree(c->d_bodies);
+    if (c->h_bodies) cudaFreeHost(c->h_bodies);
+    if (c->ev_bodies) cudaEventDestroy(c->ev_bodies);
     for (int i = 0; i < 4; ++i) if (c->cg_v[i]) cudaFree(c->cg_v[i]);
     if (c->stage_u) cudaFree(c->stage_u);
     if (c->stage_L) cudaFree(c->stage_L);
@@ -1166,8 +1172,23 @@ int wl_set_bodies(wl_ctx* c, int nbodies, const double* bodies_host) {
         cudaGetLastError();
         return fail(c, WL_ENOMEM, "wl_set_bodies: cudaMalloc");
     }
-    if (nbodies > 0)   // pageable host memory: the copy is staged before the call returns, the caller's array may be reused
-        CU(c, cudaMemcpyAsync(c->d_bodies, bodies_host, sizeof(double) * (size_t)nbodies * kBodyDoubles, cudaMemcpyHostToDevice, c->stream));
+    if (!c->h_bodies) {
+        if (cudaMallocHost((void**)&c->h_bodies, sizeof(double) * kMaxBodies * kBodyDoubles) != cudaSuccess) {
+            cudaGetLastError();
+            c->h_bodies = nullptr;
+            return fail(c, WL_ENOMEM, "wl_set_bodies: cudaMallocHost");
+        }
+        CU(c, cudaEventCreateWithFlags(&c->ev_bodies, cudaEventDisableTiming));
+    } else {
+        CU(c, cudaEventSynchronize(c->ev_bodies));   // the previous call's upload has left the staging buffer
+    }
+    if (nbodies > 0) {
+        // The records (at most 16 KB) go through a context-owned pinned buffer: with a pinned caller array the copy would be
+        // truly asynchronous and a time stepper that moves its bodies for the next step would race with it.
+        memcpy(c->h_bodies, bodies_host, sizeof(double) * (size_t)nbodies * kBodyDoubles);
+        CU(c, cudaMemcpyAsync(c->d_bodies, c->h_bodies, sizeof(double) * (size_t)nbodies * kBodyDoubles, cudaMemcpyHostToDevice, c->stream));
+    }
+    CU(c, cudaEventRecord(c->ev_bodies, c->stream));
     return DISPATCH(c, set_bodies)(c, nbodies);
 }
 
@@ -1220,11 +1241,25 @@ int wl_project(wl_ctx* c, void* u, const void* L, void* p, double tol, int maxcy
     return src;
 }
 
+static int project_host_enqueue(wl_ctx* c, void* u_host, const void* L_host, void* p_host, double tol, int maxcycles, double* hist,
+                                int* ncycles);
+
 int wl_project_host(wl_ctx* c, void* u_host, const void* L_host, void* p_host, double tol, int maxcycles, double* hist,
                     int* ncycles) {
     if (!c) return WL_EINVAL;
     if (!u_host || !p_host || !hist || !ncycles || maxcycles < 0 || !(tol >= 0.0)) return fail(c, WL_EINVAL, "wl_project_host: bad argument");
     if (!L_host && !c->have_coeff) return fail(c, WL_ESTATE, "wl_project_host: coefficients not set");
+    const int rc = project_host_enqueue(c, u_host, L_host, p_host, tol, maxcycles, hist, ncycles);
+    if (rc < 0) {   // copies from / to the caller's buffers may be in flight on either stream: the caller may free them on return
+        if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+        cudaStreamSynchronize(c->stream);
+        cudaGetLastError();
+    }
+    return rc;
+}
+
+static int project_host_enqueue(wl_ctx* c, void* u_host, const void* L_host, void* p_host, double tol, int maxcycles, double* hist,
+                                int* ncycles) {
     const size_t cell_bytes = (size_t)c->lev[0].g.M * c->esz;
     const size_t face_bytes = cell_bytes * c->n;
     if (!c->stage_u && cudaMalloc(&c->stage_u, face_bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, WL_ENOMEM, "cudaMalloc(stage_u)"); }
@@ -1314,7 +1349,10 @@ int wl_down(wl_ctx* c, int level, const void* x_in, const void* b, void* x_out, 
     if (c->opt_solve_kernels) { int rc = ensure_hist(c, 63); if (rc) return rc; }
     note_alignment(c, level, {x_in, b, x_out, bc});
     c->pdl_armed = false;
-    return DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
+    c->solve_kernels_now = c->opt_solve_kernels;
+    const int rc = DISPATCH(c, down)(c, level, x_in, b, x_out, bc ? bc : c->lev[level + 1].b);
+    c->solve_kernels_now = 0;
+    return rc;
 }
 
 int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b, void* x_out) {
@@ -1324,7 +1362,10 @@ int wl_up(wl_ctx* c, int level, const void* x_in, const void* xc, const void* b,
     if (c->opt_solve_kernels) { int rc = ensure_hist(c, 63); if (rc) return rc; }
     note_alignment(c, level, {x_in, xc, b, x_out});
     c->pdl_armed = false;
-    return DISPATCH(c, up)(c, level, x_in, xc ? xc : c->lev[level + 1].x[1], b, x_out);
+    c->solve_kernels_now = c->opt_solve_kernels;
+    const int rc = DISPATCH(c, up)(c, level, x_in, xc ? xc : c->lev[level + 1].x[1], b, x_out);
+    c->solve_kernels_now = 0;
+    return rc;
 }
 
 int wl_vcycle_level(wl_ctx* c, int level, void* x, const void* b) {
@@ -1345,6 +1386,22 @@ int wl_residual_norm(wl_ctx* c, const void* p, const void* b, double* rnorm_out,
     if ((rc = read_scalars(c))) return rc;
     *rnorm_out = bits_to_double(c->h_scal->absmax_bits[1]);
     if (mean_out) *mean_out = c->h_scal->mean_p;
+    return WL_OK;
+}
+
+int wl_selftest_recip(wl_ctx* c, uint64_t* mismatches_out, uint32_t* first_bad_bits_out) {
+    if (!c) return WL_EINVAL;
+    if (!mismatches_out) return fail(c, WL_EINVAL, "wl_selftest_recip: null pointer");
+    // slots 2 and 3 of the context's scalars are scratch: [2] = mismatch count, [3] = smallest mismatching bit pattern
+    const unsigned long long init[2] = {0ULL, ~0ULL};
+    CU(c, cudaMemcpyAsync(&c->d_scal->absmax_bits[2], init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
+    k_selftest_recip<<<c->num_sms * 16, 256, 0, c->stream>>>(0x00800000u /* 2^-126 */, 0x7E800000u /* 2^126 */, &c->d_scal->absmax_bits[2]);
+    KCHECK(c, "k_selftest_recip");
+    unsigned long long res[2] = {0, 0};
+    CU(c, cudaMemcpyAsync(res, &c->d_scal->absmax_bits[2], sizeof(res), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    *mismatches_out = res[0];
+    if (first_bad_bits_out) *first_bad_bits_out = res[0] ? (uint32_t)res[1] : 0u;
     return WL_OK;
 }
 

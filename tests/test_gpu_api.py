@@ -102,3 +102,31 @@ def test_vcycle_call_matches_oracle_cycle(env):
         assert nrm == nrm_ref
     assert p.cpu().numpy().tobytes() == p_ref.tobytes()
     pr.close()
+
+
+@pytest.mark.parametrize("config,scale", [(2, 2), (1, 4)])
+def test_solve_kernels_option_does_not_leak_into_the_solvers(env, config, scale):
+    """WL_OPT_SOLVE_KERNELS is a profiling switch of the wl_down / wl_up entry points.  With it set (and the solve history
+    allocated by an earlier solve) wl_vcycle, the plain wl_solve and wl_solve_pcg must still run their own kernel instances:
+    the solve instances subtract a stale mean on load and bump the cycle counter."""
+    torch, wl = env["torch"], env["wl"]
+    cfg, o, b, pr = _case(env, config, scale)
+    bd = torch.from_numpy(b).cuda()
+    p = torch.zeros(b.shape, dtype=torch.float32, device="cuda")
+    wl.wl_solve(pr.ctx, p, bd, 0.0, 3)                                   # allocates the history, leaves a non-zero shift behind
+    wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 1)
+    p0 = np.random.default_rng(9).standard_normal(b.shape).astype(np.float32) + np.float32(2.0)
+    p_ref, r_ref = o.vcycle(p0, b)
+    p1 = torch.from_numpy(p0).cuda()
+    r1 = wl.wl_vcycle(pr.ctx, p1, bd)
+    assert np.abs(p1.cpu().numpy() - p_ref).max() <= 1e-4 * np.abs(p_ref).max()
+    assert abs(r1 / r_ref - 1) <= 1e-3
+    wl.wl_set_option(pr.ctx, wl.WL_OPT_GRAPH, 0)                         # the non-lagged, non-graph solve calls down()/up() too
+    for solver, ref in ((wl.wl_solve, o.solve), (wl.wl_solve_pcg, o.solve_pcg)):
+        p_ref, hist_ref, nc_ref, rc_ref = ref(np.zeros_like(b), b, 0.0, 4)
+        p2 = torch.zeros(b.shape, dtype=torch.float32, device="cuda")
+        hist, nc, rc = solver(pr.ctx, p2, bd, 0.0, 4)
+        assert (nc, rc) == (nc_ref, rc_ref)
+        assert np.abs(hist / hist_ref - 1).max() <= 1e-3, (hist, hist_ref)
+        assert np.abs(p2.cpu().numpy() - p_ref).max() <= 1e-4 * np.abs(p_ref).max()
+    pr.close()

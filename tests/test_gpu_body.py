@@ -120,3 +120,27 @@ def test_moving_body_projection_matches_the_oracle(env):
         assert np.abs(p.cpu().numpy() - p_ref).max() <= 1e-4 * np.abs(p_ref).max()
         assert np.abs(ud.cpu().numpy() - u_ref).max() <= 1e-4 * np.abs(u_ref).max()
     pr.close()
+
+
+def test_config4_full_512_thirty_two_spheres(env):
+    """wl_set_bodies at the size and body count bench.py's `e2e` leg runs it on every step (BASELINE configs[4]: 512^3 fp32, 32
+    seeded spheres; Table 2 `BDIM!`): level 0 against oracle.body_coeff face by face, every coarse level
+    bit-exact against the oracle's coarsening of the GPU's own level 0."""
+    torch, wl, o = env["torch"], env["wl"], env["oracle"]
+    dt = np.float32
+    cfg = env["synth"].make_config(4, dtype=dt)
+    dims = cfg["dims"]
+    rec = _bodies_of(env, 4, dims, 1)
+    assert rec.shape == (32, 8) and int(np.prod(dims)) == 512 ** 3
+    Lo = o.body_coeff(dims, dt, rec)
+    assert np.array_equal(Lo, cfg["L"])
+    pr = wl.Projector(dims, dt)
+    wl.wl_set_bodies(pr.ctx, rec)
+    Lg = pr.get_coeff(0).cpu().numpy()
+    _check_level0(Lg, Lo, dt)
+    del Lo
+    orc = o.Oracle(dims, dt)
+    orc.set_coeff(Lg)
+    for l in range(pr.num_levels):
+        assert pr.get_coeff(l).cpu().numpy().tobytes() == orc.get_coeff(l).tobytes(), l
+    pr.close()
