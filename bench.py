@@ -81,7 +81,8 @@ def csrc_hash() -> str:
     import glob
     import hashlib
     h = hashlib.sha256()
-    files = sorted(glob.glob(os.path.join(ROOT, "paper_2304_08159_b200", "csrc", "*.cu*"))) + [os.path.join(ROOT, "include", "wl.h")]
+    csrc = os.path.join(ROOT, "paper_2304_08159_b200", "csrc")
+    files = sorted(glob.glob(os.path.join(csrc, "*.cu*")) + glob.glob(os.path.join(csrc, "*.h"))) + [os.path.join(ROOT, "include", "wl.h")]
     for f in files:
         with open(f, "rb") as fh:
             h.update(os.path.basename(f).encode() + b"\0" + fh.read())
@@ -233,6 +234,7 @@ def main():
     ap.add_argument("--e2e-upload-L", action="store_true", help="e2e leg: upload the n·M coefficient array instead of the body records")
     ap.add_argument("--no-pcg", action="store_true", help="skip the conjugate-gradient leg (reported beside the V-cycle solver)")
     ap.add_argument("--no-convdiff", action="store_true", help="skip the convdiff leg (NEXT-4, timed alone on the same velocity)")
+    ap.add_argument("--no-vcycle-256", action="store_true", help="skip the 256^3 V-cycle leg that rides on the default config-4 run")
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--graph", type=int, default=1)
     ap.add_argument("--pdl", type=int, default=1, help="WL_OPT_PDL: programmatic dependent launch between the kernels of a cycle")
@@ -308,36 +310,70 @@ def main():
         barrier()
         total_ms = float(np.sum(ms))
 
-        # the dominant kernels alone (roofline leg), straight after the timed steps
-        kern = {}
+        # the dominant kernels alone (roofline leg): first straight after the timed steps, with the board in the power / clock
+        # state a long step leaves it in ("in_step"), then again after a short idle ("burst": MEASURED_PEAKS.json's copy rate
+        # is a burst figure — a copy kernel timed alone on an idle GPU — so that is the like-for-like fraction).
+        kern, kern_in_step = {}, {}
         reps = max(5, args.kernel_reps)
         if pr.num_levels > 1:
-            # MEASURED_PEAKS.json's copy rate is a burst figure (a copy kernel timed alone on an idle GPU); the kernel is timed the
-            # same way: alone, after a short idle that lets the board leave the power-capped state the timed steps put it in
-            # (the in-step cost of the same kernels is what `vcycle` and `ms_per_step` report).
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 1)   # time the instances the solve's graph launches
+            bd = pr.empty_cells()
+            wl.wl_divergence(pr.ctx, u0, bd)
+            xo = pr.empty_cells()
+
+            def time_level0(out):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                for name, fn in (("down", lambda: wl.wl_down(pr.ctx, 0, p, bd, xo)),
+                                 ("up", lambda: wl.wl_up(pr.ctx, 0, xo, None, bd, p))):
+                    for _ in range(3):
+                        fn()
+                    l0 = wl.wl_launch_count(pr.ctx)
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    for _ in range(reps):
+                        fn()
+                    e1.record(stream)
+                    e1.synchronize()
+                    out[name] = {"ms": e0.elapsed_time(e1) / reps, "launches_per_call": (wl.wl_launch_count(pr.ctx) - l0) // reps}
+
+            for _ in range(2):                      # two more projections so the kernels below start from the step's own state
+                one_step()
+            time_level0(kern_in_step)
             torch.cuda.synchronize()
             clk.paused = True
             time.sleep(args.roofline_idle)
             clk.paused = False
-            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 1)   # time the instances the solve's graph launches
-            bd = pr.empty_cells()
-            wl.wl_divergence(pr.ctx, u0, bd)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            xo = pr.empty_cells()
-            for name, fn in (("down", lambda: wl.wl_down(pr.ctx, 0, p, bd, xo)),
-                             ("up", lambda: wl.wl_up(pr.ctx, 0, xo, None, bd, p))):
-                for _ in range(3):
-                    fn()
-                l0 = wl.wl_launch_count(pr.ctx)
+            time_level0(kern)
+            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 0)
+            del xo
+
+        # where the part of ms_per_step that is not V-cycles goes: the pieces of one projection timed one by one through their
+        # own entry points (same kernels; wl_solve = cycles + the final mean shift)
+        breakdown = None
+        if pr.num_levels > 1:
+            def timed(fn, nrep=3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                fn()
                 torch.cuda.synchronize()
                 e0.record(stream)
-                for _ in range(reps):
+                for _ in range(nrep):
                     fn()
                 e1.record(stream)
                 e1.synchronize()
-                kern[name] = {"ms": e0.elapsed_time(e1) / reps, "launches_per_call": (wl.wl_launch_count(pr.ctx) - l0) // reps}
-            wl.wl_set_option(pr.ctx, wl.WL_OPT_SOLVE_KERNELS, 0)
-            del xo
+                return e0.elapsed_time(e1) / nrep
+            bq = pr.empty_cells()
+            u.copy_(u0)
+            breakdown = {"set_coeff": timed(lambda: wl.wl_set_coeff(pr.ctx, Ld)),
+                         "divergence": timed(lambda: wl.wl_divergence(pr.ctx, u, bq))}
+            def solve_once():
+                p.zero_()
+                return wl.wl_solve(pr.ctx, p, bq, tol, maxc)
+            breakdown["solve"] = timed(solve_once, 2)
+            breakdown["solve_cycles"] = int(solve_once()[1])
+            breakdown["gradient"] = timed(lambda: wl.wl_gradient(pr.ctx, u, p))
+            breakdown["sum"] = breakdown["set_coeff"] + breakdown["divergence"] + breakdown["solve"] + breakdown["gradient"]
+            breakdown["note"] = "ms; solve includes p.zero_() and the final mean shift; pieces timed alone, so their sum need not equal ms_per_step"
+            del bq
 
         # e2e: the same projection through the host-buffer entry point with pinned HOST buffers.  Inputs of a step: the
         # face velocity u (n·M values) and the bodies' analytic description (8 doubles each) from which wl_set_bodies builds
@@ -411,6 +447,34 @@ def main():
         e1.synchronize()
         vcycle_ms = e0.elapsed_time(e1) / reps
 
+        # the other grid BASELINE.json's target names (256^3 fp32, config 3): V-cycles alone on a context of its own (0.3 GB)
+        vc256 = None
+        if world == 1 and not args.donut and args.config == 4 and args.scale == 1 and not args.no_vcycle_256:
+            c3 = synth.make_config(3)
+            d3, M3, n3, es3 = c3["dims"], int(np.prod(c3["dims"])), len(c3["dims"]), c3["dtype"].itemsize
+            pr3 = wl.Projector(d3, c3["dtype"], dev)
+            wl.wl_set_option(pr3.ctx, wl.WL_OPT_PDL, args.pdl)
+            wl.wl_set_coeff(pr3.ctx, torch.from_numpy(c3["L"]).to(dev))
+            b3, p3 = pr3.empty_cells(), pr3.zeros_cells()
+            wl.wl_divergence(pr3.ctx, torch.from_numpy(c3["u"]).to(dev), b3)
+            wl.wl_solve(pr3.ctx, p3, b3, 0.0, 3)
+            best = None
+            for _ in range(3):
+                p3.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record(stream)
+                wl.wl_solve(pr3.ctx, p3, b3, 0.0, reps)
+                e1.record(stream)
+                e1.synchronize()
+                t3 = e0.elapsed_time(e1) / reps
+                best = t3 if best is None else min(best, t3)
+            eff3 = (2 * (n3 + 3) + 2.0 / 2 ** n3) * es3 * (2 ** n3 / (2 ** n3 - 1.0)) * M3 / (best * 1e-3) / 1e9
+            vc256 = {"workload": c3["name"], "ms": best, "effective_GBps_56B_model": eff3, "frac_of_measured": eff3 / _peaks()[0],
+                     "frac_of_nominal_8TBs": eff3 / NOMINAL_HBM_GBS, "timed": f"best of 3 x {reps} cycles (wl_solve, tol = 0); working set fits L2"}
+            pr3.close()
+            del b3, p3
+
     clocks = clk.summary()
 
     # max over ranks
@@ -437,7 +501,13 @@ def main():
                 "traffic": recorded_traffic(cfg["name"], "down"),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_down,
                 "launches_per_call": kern["down"]["launches_per_call"], "ms": kern["down"]["ms"],
-                "timed": f"{reps} launches alone after 3 warm-ups and {args.roofline_idle} s of idle (burst, as the peak was measured)",
+                "timed": f"{reps} launches alone after 3 warm-ups and {args.roofline_idle} s of idle (burst, as the peak was measured); "
+                         "in_step = the same launches straight after the timed projections, no idle",
+                "in_step": {"ms": kern_in_step["down"]["ms"],
+                            "achieved": bytes_down / (kern_in_step["down"]["ms"] * 1e-3) / 1e9,
+                            "frac": bytes_down / (kern_in_step["down"]["ms"] * 1e-3) / 1e9 / peak,
+                            "up_ms": kern_in_step["up"]["ms"],
+                            "up_frac": bytes_down / (kern_in_step["up"]["ms"] * 1e-3) / 1e9 / peak},
                 "up_kernel": {"ms": kern["up"]["ms"], "achieved": bytes_down / (kern["up"]["ms"] * 1e-3) / 1e9,
                               "frac": bytes_down / (kern["up"]["ms"] * 1e-3) / 1e9 / peak,
                               "traffic": recorded_traffic(cfg["name"], "up"),
@@ -454,6 +524,8 @@ def main():
         "vcycle": (lambda eff: {"ms": vcycle_ms, "cells_per_s": M / (vcycle_ms * 1e-3), "effective_GBps_56B_model": eff,
                                 "frac_of_measured": eff / peak, "frac_of_nominal_8TBs": eff / NOMINAL_HBM_GBS})(
             (2 * (n + 3) + 2.0 / 2 ** n) * esz * (2 ** n / (2 ** n - 1.0)) * M / (vcycle_ms * 1e-3) / 1e9),
+        "vcycle_256": vc256,
+        "breakdown_ms": breakdown,
         "pcg": pcg,
         "convdiff": convdiff_report(cd, n, M, esz, peak, clocks),
         "gpu_launches": int(launches),

@@ -32,7 +32,7 @@ def _sources():
 
 def _deps():
     inc = os.path.join(os.path.dirname(HERE), "include", "wl.h")
-    return _sources() + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [inc]
+    return _sources() + sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h"))) + [inc]
 
 
 def needs_build() -> bool:

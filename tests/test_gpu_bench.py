@@ -28,3 +28,8 @@ def test_bench_prints_the_contract_line():
     cd = line["convdiff"]
     assert cd["roofline"]["bound"] == "alu" and cd["ms"] > 0 and cd["cpu_baseline"]["value"] > 0
     assert line["config"]["converged"] is True and line["pcg"]["converged"] is True
+    # the level-0 kernels timed in the state the timed steps leave the board in, beside the burst figure; where the rest of a step goes
+    assert r["in_step"]["ms"] > 0 and abs(r["in_step"]["frac"] - r["in_step"]["achieved"] / r["peak"]) < 1e-9
+    bd = line["breakdown_ms"]
+    assert all(bd[k] > 0 for k in ("set_coeff", "divergence", "solve", "gradient")) and bd["solve_cycles"] == line["config"]["cycles_run"]
+    assert line["vcycle_256"] is None            # rides on the default config-4 run only
