@@ -167,8 +167,10 @@ def _algorithmic_bytes_down(n: int, esz: int) -> float:
 # bound (3), two medians (8 compare/select), flux (4) = 22 operations; 9 fluxes per 3-D cell (each face flux serves two control
 # volumes) + 2 per flux difference accumulated x 9 = 216 operations per cell (2-D: 4 fluxes, 96).  None can fuse into an FMA
 # (every operation rounds separately, reading 12), so the ALU ceiling is one operation per FP32 lane and clock:
-# SMs x 128 lanes x SM clock (B200_PROFILING.md: 148 SMs; the clock is the one sampled during the run).
-def convdiff_report(cd, n, M, esz, hbm_peak, clocks):
+# SMs x 128 lanes x SM clock (B200_PROFILING.md: 148 SMs; the clock is the one sampled during the run).  The packed f32x2
+# instructions the kernel uses do not raise that ceiling: wl_selftest_fp32_rates measures 128 lane-operations per clock and SM
+# for scalar and packed adds and fmas alike (profiles/r3_packed_rate.md); the measured figure rides along as `alu_rates`.
+def convdiff_report(cd, n, M, esz, hbm_peak, clocks, rates=None):
     if cd is None:
         return None
     sec = cd["ms"] * 1e-3
@@ -180,7 +182,8 @@ def convdiff_report(cd, n, M, esz, hbm_peak, clocks):
     return {"kernel": "k_convdiff3d (TMA-staged tiles, every flux once)" if n == 3 else "k_convdiff (one thread per cell)",
             "ms": cd["ms"], "cells_per_s": M / sec,
             "roofline": {"bound": "alu", "achieved": ops / sec / 1e12, "peak": alu_peak, "unit": "TFLOP/s", "frac": ops / sec / 1e12 / alu_peak,
-                         "ops_per_cell": ops // M, "peak_source": f"148 SMs x {lanes} lanes x sampled SM clock ({mhz} MHz), one non-fused operation per lane and clock"},
+                         "ops_per_cell": ops // M, "peak_source": f"148 SMs x {lanes} lanes x sampled SM clock ({mhz} MHz), one non-fused operation per lane and clock",
+                         "alu_rates": None if rates is None else {k: {"warp_instr_per_clk_sm": v[0], "lane_ops_per_clk_sm": v[1]} for k, v in rates.items()}},
             "hbm": {"algorithmic_bytes": nb, "achieved_GBps": nb / sec / 1e9, "frac_of_measured": nb / sec / 1e9 / hbm_peak}}
 
 
@@ -416,7 +419,7 @@ def main():
                    "ms_per_projection": float(np.mean(pms)), "final_rel_residual": float(hp[-1] / hp[0]) if hp[0] > 0 else 0.0}
 
         # NEXT-4: the other dominant routine of the paper's step (`convdiff!`) on the same velocity field, timed alone
-        cd = None
+        cd, fp32_rates = None, None
         if not args.no_convdiff:
             rcd = torch.empty_like(u0)
             for _ in range(3):
@@ -430,6 +433,7 @@ def main():
             e1.synchronize()
             cd = {"ms": e0.elapsed_time(e1) / reps}
             del rcd
+            fp32_rates = wl.wl_selftest_fp32_rates(pr.ctx)   # measured lane-operations per clock and SM, scalar and packed
 
         # V-cycles alone: wl_solve with tol = 0 runs exactly `reps` cycles (one graph launch + one 8-byte readback each,
         # mean shift deferred into the next cycle); the dominant kernels alone follow
@@ -527,7 +531,7 @@ def main():
         "vcycle_256": vc256,
         "breakdown_ms": breakdown,
         "pcg": pcg,
-        "convdiff": convdiff_report(cd, n, M, esz, peak, clocks),
+        "convdiff": convdiff_report(cd, n, M, esz, peak, clocks, fp32_rates),
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": roof,

@@ -48,6 +48,7 @@ SIGNATURES = {
     "wl_residual_norm_static": (_i32, [_i32, _i64p, _i32, _vp, _vp, _vp, _vp, _vp]),
     "wl_static_last_error": (ctypes.c_char_p, []),
     "wl_selftest_recip": (_i32, [_vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint32)]),
+    "wl_selftest_fp32_rates": (_i32, [_vp, _f64p]),
     "wl_num_levels": (_i32, [_vp]),
     "wl_level_dims": (_i32, [_vp, _i32, _i64p]),
     "wl_get_coeff": (_i32, [_vp, _i32, _vp]),
@@ -250,6 +251,14 @@ def wl_selftest_recip(ctx):
     n, first = ctypes.c_uint64(0), ctypes.c_uint32(0)
     _check(ctx, load().wl_selftest_recip(ctx, ctypes.byref(n), ctypes.byref(first)), "wl_selftest_recip")
     return int(n.value), int(first.value)
+
+
+def wl_selftest_fp32_rates(ctx) -> dict:
+    """Measured fp32 issue and arithmetic rates per clock and SM: {variant: (warp_instr_per_clk, lane_ops_per_clk)}."""
+    out = (ctypes.c_double * 8)()
+    _check(ctx, load().wl_selftest_fp32_rates(ctx, out), "wl_selftest_fp32_rates")
+    names = ("add.f32", "add.f32x2", "fma.f32", "fma.f32x2")
+    return {nm: (out[2 * i], out[2 * i + 1]) for i, nm in enumerate(names)}
 
 
 WL_STATIC_MAX_CELLS = 1 << 27

@@ -23,10 +23,20 @@
 #include "wl_pcg.cuh"
 #include "wl_body.cuh"
 #include "wl_convdiff.cuh"
+#include "wl_rates.cuh"
 
 using namespace wl;
 
 namespace {
+
+// fp64 fused 3-D kernels: 1 (default) = read omega/D as a precomputed sixth plane, 0 = recompute it from the coefficients with an
+// IEEE division, as the fp32 kernels do with their reciprocal.  A/B switch (build.py: WL_NVCC_EXTRA=-DWL_FP64_C_PLANE=0).  Measured
+// at 256^3 on a B200 (round 3): recomputing saves 134 MB of DRAM traffic per launch but costs more than it saves — level-0 DOWN
+// 0.280 ms against 0.242 ms with the plane (the division's ~20 dependent FP64 instructions, a few spilled registers), UP unchanged
+// at 0.250 ms, V-cycle 0.696 against 0.643 ms — so the plane stays.
+#ifndef WL_FP64_C_PLANE
+#define WL_FP64_C_PLANE 1
+#endif
 
 constexpr int kMaxLevels = 32;
 constexpr int kBlock = 256;
@@ -304,7 +314,7 @@ struct Impl {
     // the kernel (5 planes per ring slot); fp64: 32x14 cells, omega/D read as a sixth plane (an IEEE fp64 division is ~20
     // instructions).  12 warps each.  Measured alternatives: profiles/r2_fused_ncu.md.
     static constexpr int FTX = sizeof(T) == 4 ? 64 : 32, FTY = sizeof(T) == 4 ? 16 : 14;
-    static constexpr bool USEC = sizeof(T) == 8;
+    static constexpr bool USEC = sizeof(T) == 8 && WL_FP64_C_PLANE != 0;
     template <bool PROLONG> static constexpr int FPF = (PROLONG && USEC) ? 2 : 3;   // fp32 DOWN with 4 planes in flight: no gain
 
     // Fused kernels apply to 3-D levels that have a coarser level, whose rows (and the coarse rows) are whole 16-byte
@@ -1055,7 +1065,7 @@ int wl_create(int ndim, const int64_t* dims, int dtype, wl_ctx** out) {
     for (int l = 0; l < nlev; ++l) {
         Level& v = c->lev[l];
         dmalloc(&v.L, (size_t)v.g.M * ndim * c->esz);
-        if (dtype == WL_F64 && ndim == 3) dmalloc(&v.C, (size_t)v.g.M * c->esz);   // read by the fp64 fused kernels only
+        if (WL_FP64_C_PLANE && dtype == WL_F64 && ndim == 3) dmalloc(&v.C, (size_t)v.g.M * c->esz);   // read by the fp64 fused kernels only
         dmalloc(&v.x[1], (size_t)v.g.M * c->esz);
         if (l > 0) {
             dmalloc(&v.x[0], (size_t)v.g.M * c->esz);
@@ -1402,6 +1412,39 @@ int wl_selftest_recip(wl_ctx* c, uint64_t* mismatches_out, uint32_t* first_bad_b
     CU(c, cudaStreamSynchronize(c->stream));
     *mismatches_out = res[0];
     if (first_bad_bits_out) *first_bad_bits_out = res[0] ? (uint32_t)res[1] : 0u;
+    return WL_OK;
+}
+
+int wl_selftest_fp32_rates(wl_ctx* c, double* out8) {
+    if (!c) return WL_EINVAL;
+    if (!out8) return fail(c, WL_EINVAL, "wl_selftest_fp32_rates: null pointer");
+    // clocks of the timed loop per CTA land in the context's partials array (one CTA per SM, 16 warps each)
+    constexpr int kWarps = 16, kIters = 4096;
+    const int ctas = c->num_sms < kMaxPartials ? c->num_sms : kMaxPartials;
+    long long* cyc = (long long*)c->d_partials;
+    float* sink = (float*)&c->d_scal->absmax_bits[2];
+    std::vector<long long> h((size_t)ctas);
+    for (int mode = 0; mode < 4; ++mode) {
+        for (int pass = 0; pass < 2; ++pass) {   // first pass warms the instruction cache
+            const int it = pass ? kIters : 16;
+            switch (mode) {
+                case 0: k_fp32_rate<0><<<ctas, kWarps * 32, 0, c->stream>>>(sink, cyc, it, 1.0f); break;
+                case 1: k_fp32_rate<1><<<ctas, kWarps * 32, 0, c->stream>>>(sink, cyc, it, 1.0f); break;
+                case 2: k_fp32_rate<2><<<ctas, kWarps * 32, 0, c->stream>>>(sink, cyc, it, 1.0f); break;
+                default: k_fp32_rate<3><<<ctas, kWarps * 32, 0, c->stream>>>(sink, cyc, it, 1.0f); break;
+            }
+            KCHECK(c, "k_fp32_rate");
+        }
+        CU(c, cudaMemcpyAsync(h.data(), cyc, sizeof(long long) * (size_t)ctas, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        double avg = 0.0;
+        for (int i = 0; i < ctas; ++i) avg += (double)h[(size_t)i];
+        avg /= ctas;
+        const bool packed = (mode & 1) != 0;
+        const double winstr = (double)kWarps * kIters * (packed ? 8 : 16);
+        out8[2 * mode] = winstr / avg;                               // warp-instructions per clock and SM
+        out8[2 * mode + 1] = winstr * 32.0 * (packed ? 2 : 1) / avg;   // lane-operations (an fma counted once) per clock and SM
+    }
     return WL_OK;
 }
 
